@@ -1,0 +1,336 @@
+"""Pins for the CPU oracle (oracle/jdft_ref.c): each test checks it against something OTHER than itself --
+brute-force definitions, closed forms, invariants the formulation fixes (BASELINE.json
+north_star), and the exact basis sizes in tests/golden/basis_counts.txt.
+All CPU-only ("-m 'not gpu'").  A plausible mistake in the oracle (dropped term, wrong sign, wrong index
+order, transposed operand, missing Omega or 1/N) fails at least one of these.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _rand_c(rng, *shape):
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+def _skew_lattice():
+    # non-orthogonal cell, columns are lattice vectors
+    return np.array([[5.0, 0.7, -0.4], [0.3, 6.0, 0.9], [-0.5, 0.2, 7.0]])
+
+
+def _brute_I_matrix(b):
+    """Explicit N x nG matrix exp(+2 pi i sum_d iG[n]_d j_d / S_d), j in row-major box order."""
+    S = b.shape
+    j = np.stack(np.meshgrid(np.arange(S[0]), np.arange(S[1]), np.arange(S[2]), indexing="ij"), -1).reshape(-1, 3)
+    phase = (j[:, None, :] * b.iG[None, :, :].astype(np.float64) / np.asarray(S, dtype=np.float64)).sum(-1)
+    return np.exp(2j * np.pi * phase)
+
+
+# ------------------------------------------------------------------------------------------ 1-D FFT
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 7, 8, 9, 10, 12, 15, 25, 27, 30, 32, 45, 60, 72, 80, 125, 128, 216])
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_fft1d_vs_bruteforce_dft(ref, n, sign):
+    rng = np.random.default_rng(n * 7 + sign)
+    x = _rand_c(rng, n)
+    jq = (np.arange(n)[:, None] * np.arange(n)[None, :]) % n
+    W = np.exp(sign * 2j * np.pi * jq.astype(np.longdouble) / n).astype(np.clongdouble)
+    want = (W @ x.astype(np.clongdouble)).astype(np.complex128)
+    got = ref.fft1d(x, sign)
+    assert np.max(np.abs(got - want)) <= 1e-13 * np.sqrt(n) * np.max(np.abs(want))
+
+
+def test_fft1d_delta_and_constant(ref):
+    n = 60
+    x = np.zeros(n, complex); x[7] = 1.0
+    got = ref.fft1d(x, +1)
+    assert np.allclose(got, np.exp(2j * np.pi * 7 * np.arange(n) / n), atol=1e-15)
+    got = ref.fft1d(np.ones(n, complex), -1)
+    want = np.zeros(n, complex); want[0] = n
+    assert np.allclose(got, want, atol=1e-13)
+
+
+# ------------------------------------------------------------------------------------------ basis
+
+def _golden_counts():
+    rows = []
+    with open(os.path.join(GOLDEN, "basis_counts.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                rows.append([int(t) for t in line.split()])
+    return rows
+
+
+@pytest.mark.parametrize("row", _golden_counts(), ids=lambda r: "cfg%d_k%d" % (r[0], r[1]))
+def test_basis_exact_counts_and_extents(ref, row):
+    cfg, ik, nG, *ext = row
+    R, kpts, Ecut, S = workloads.lattice(cfg)
+    b = ref.RefBasis(R, kpts[ik], Ecut, S)
+    assert b.nG == nG
+    got = [b.iG[:, 0].min(), b.iG[:, 0].max(), b.iG[:, 1].min(), b.iG[:, 1].max(), b.iG[:, 2].min(), b.iG[:, 2].max()]
+    assert got == ext
+    # continuum estimate Omega (2 Ecut)^{3/2} / (6 pi^2) within 0.5 %
+    cont = b.volume * (2 * Ecut) ** 1.5 / (6 * np.pi ** 2)
+    assert abs(b.nG - cont) / cont < 5e-3
+
+
+def test_basis_bruteforce_order_index_and_symmetry(ref):
+    R = _skew_lattice()
+    S = (12, 15, 16)
+    for k in ([0.0, 0.0, 0.0], [0.25, -0.1, 0.4]):
+        Ecut = 6.0
+        b = ref.RefBasis(R, k, Ecut, S)
+        # independent evaluation through CARTESIAN q = G^T (m + k) with numpy's inverse
+        G = 2 * np.pi * np.linalg.inv(R)
+        rng_ = [np.arange(-(s // 2), (s + 1) // 2) for s in S]
+        m = np.stack(np.meshgrid(*rng_, indexing="ij"), -1).reshape(-1, 3)   # lexicographic, m2 fastest
+        q = (m + np.asarray(k)) @ G                                           # rows: G^T (m+k)
+        ke = 0.5 * (q * q).sum(1)
+        keep = ke < Ecut
+        assert b.nG == keep.sum()
+        assert np.array_equal(b.iG, m[keep].astype(np.int32))
+        assert np.allclose(b.ke, ke[keep], rtol=1e-13, atol=0)
+        mm = m[keep] % np.asarray(S)
+        assert np.array_equal(b.index, ((mm[:, 0] * S[1] + mm[:, 1]) * S[2] + mm[:, 2]).astype(np.int32))
+        assert len(np.unique(b.index)) == b.nG
+        if not any(k):
+            have = {tuple(t) for t in b.iG.tolist()}
+            assert all((-a, -bb, -c) in have for (a, bb, c) in have)   # Gamma: m in B <=> -m in B
+    assert np.isclose(b.volume, abs(np.linalg.det(R)), rtol=1e-14)
+
+
+def test_basis_cubic_gamma_closed_form_ke(ref):
+    L = 10.0
+    b = ref.RefBasis(np.diag([L, L, L]), [0, 0, 0], 10.0, (32, 32, 32))
+    m2 = (b.iG.astype(np.int64) ** 2).sum(1)
+    assert np.allclose(b.ke, 0.5 * (2 * np.pi / L) ** 2 * m2, rtol=1e-14)
+    assert np.all(b.ke < 10.0) and b.nG == np.sum(0.5 * (2 * np.pi / L) ** 2 * ((np.indices((33, 33, 33)) - 16) ** 2).sum(0) < 10.0)
+
+
+def test_volumes(ref):
+    want = {1: 1000.0, 2: 8615.125, 3: 27000.0, 4: 24000.0, 5: 28934.443}
+    for cfg, vol in want.items():
+        R, kpts, Ecut, S = workloads.lattice(cfg)
+        assert np.isclose(abs(np.linalg.det(R)), vol, rtol=1e-12)
+    b = ref.RefBasis(np.diag([20.5] * 3), [0.25] * 3, 2.0, (20, 20, 20))
+    assert np.isclose(b.volume, 8615.125, rtol=1e-14)
+
+
+def test_basis_errors(ref):
+    with pytest.raises(ref.RefError):      # 7 is not 2,3,5-smooth
+        ref.RefBasis(np.eye(3) * 10, [0, 0, 0], 5.0, (14, 16, 16))
+    with pytest.raises(ref.RefError):      # sphere wider than the box -> collision
+        ref.RefBasis(np.eye(3) * 10, [0, 0, 0], 10.0, (8, 32, 32))
+
+
+# ------------------------------------------------------------------------------------------ I, Idag, J
+
+@pytest.mark.parametrize("S,k,R,Ecut", [((8, 8, 8), (0, 0, 0), np.eye(3) * 7.0, 3.0),
+                                        ((4, 6, 5), (0.3, -0.2, 0.1), _skew_lattice(), 1.6),
+                                        ((8, 9, 10), (0.5, 0.25, -0.125), _skew_lattice() * 1.3, 2.5)])
+def test_I_Idag_vs_explicit_matrix(ref, S, k, R, Ecut):
+    b = ref.RefBasis(R, k, Ecut, S)
+    assert b.nG > 12
+    rng = np.random.default_rng(11)
+    E = _brute_I_matrix(b)
+    C = _rand_c(rng, 3, b.nG)
+    psi = b.apply_I(C).reshape(3, -1)
+    want = C @ E.T
+    assert np.max(np.abs(psi - want)) <= 1e-12 * np.max(np.abs(want))
+    f = _rand_c(rng, 2, b.N)
+    got = b.apply_Idag(f)
+    want = f @ E.conj()
+    assert np.max(np.abs(got - want)) <= 1e-12 * np.max(np.abs(want))
+    assert np.allclose(b.apply_J(f), want / b.N, rtol=0, atol=1e-13 * np.max(np.abs(want)))
+
+
+def test_I_matches_numpy_ifftn(ref):
+    R, kpts, Ecut, S = workloads.lattice(1)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    rng = np.random.default_rng(5)
+    C = _rand_c(rng, 2, b.nG)
+    box = np.zeros((2, b.N), complex)
+    box[:, b.index] = C
+    want = np.fft.ifftn(box.reshape((2,) + b.shape), axes=(1, 2, 3)) * b.N
+    got = b.apply_I(C)
+    assert np.max(np.abs(got - want)) <= 1e-13 * np.max(np.abs(want))
+
+
+def test_JI_identity_IJ_idempotent_parseval_adjoint(ref):
+    R = _skew_lattice() * 2.0
+    b = ref.RefBasis(R, [0.2, 0.1, -0.3], 5.0, (24, 30, 32))
+    rng = np.random.default_rng(3)
+    C = _rand_c(rng, 3, b.nG)
+    psi = b.apply_I(C)
+    # J I = 1 ("and vice versa")
+    assert np.max(np.abs(b.apply_J(psi) - C)) <= 1e-13 * np.max(np.abs(C))
+    # Parseval: sum_j |psi|^2 = N sum_n |C|^2
+    assert np.allclose((np.abs(psi) ** 2).sum(axis=(1, 2, 3)), b.N * (np.abs(C) ** 2).sum(1), rtol=1e-13)
+    # I J is idempotent
+    f = _rand_c(rng, 2, b.N)
+    g = b.apply_I(b.apply_J(f))
+    g2 = b.apply_I(b.apply_J(g))
+    assert np.max(np.abs(g2 - g)) <= 1e-13 * np.max(np.abs(g))
+    # adjointness <f, I C> = <Idag f, C>
+    lhs = np.vdot(f[0], psi[0].reshape(-1))
+    rhs = np.vdot(b.apply_Idag(f[:1])[0], C[0])
+    assert abs(lhs - rhs) <= 1e-13 * abs(lhs)
+
+
+def test_cos_potential_closed_form_sign_and_wrap(ref):
+    """V[j] = cos(2 pi mv.j/S) => Idag(V .* I e_m) = (N/2)(e_{m+mv} + e_{m-mv}) restricted to the sphere."""
+    R, kpts, Ecut, S = workloads.lattice(101)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    mv = np.array([1, -2, 1])
+    j = np.stack(np.meshgrid(*[np.arange(s) for s in S], indexing="ij"), -1)
+    V = np.cos(2 * np.pi * (j * mv / np.asarray(S)).sum(-1))
+    lookup = {tuple(m): n for n, m in enumerate(b.iG.tolist())}
+    for n0 in (0, b.nG // 2, b.nG - 1):
+        C = np.zeros((1, b.nG), complex); C[0, n0] = 1.0
+        got = b.apply_Idag(V[None] * b.apply_I(C))[0]
+        want = np.zeros(b.nG, complex)
+        for sgn in (+1, -1):
+            t = tuple((b.iG[n0] + sgn * mv).tolist())
+            if t in lookup:
+                want[lookup[t]] += 0.5 * b.N
+        assert np.max(np.abs(got - want)) <= 1e-12 * b.N
+        # an asymmetric (complex) potential exp(+2 pi i mv.j/S) must shift m -> m + mv, not m - mv
+        Vc = np.exp(2j * np.pi * (j * mv / np.asarray(S)).sum(-1))
+        got = b.apply_Idag(Vc[None] * b.apply_I(C))[0]
+        want = np.zeros(b.nG, complex)
+        t = tuple((b.iG[n0] + mv).tolist())
+        if t in lookup:
+            want[lookup[t]] = b.N
+        assert np.max(np.abs(got - want)) <= 1e-12 * b.N
+
+
+# ------------------------------------------------------------------------------------------ L, O, overlap
+
+def test_L_O_closed_forms(ref):
+    R = _skew_lattice()
+    k = np.array([0.1, 0.2, -0.3])
+    b = ref.RefBasis(R, k, 5.0, (16, 18, 20))
+    rng = np.random.default_rng(9)
+    C = _rand_c(rng, 2, b.nG)
+    G = 2 * np.pi * np.linalg.inv(R)
+    q = (b.iG + k) @ G
+    q2 = (q * q).sum(1)
+    vol = abs(np.linalg.det(R))
+    assert np.allclose(b.apply_L(C), -vol * q2[None, :] * C, rtol=1e-13)
+    assert np.allclose(b.apply_O(C), vol * C, rtol=1e-15)
+
+
+def test_overlap_orthonormal_bands_and_library_gemm(ref):
+    cfg = 102
+    R, kpts, Ecut, S = workloads.lattice(cfg)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    C = workloads.make_bands(cfg, b.nG)
+    M = b.overlap(C, C)
+    assert np.max(np.abs(M - np.eye(C.shape[0]))) <= 1e-13           # generator: C^+ O C = 1
+    rng = np.random.default_rng(2)
+    C1, C2 = _rand_c(rng, 4, b.nG), _rand_c(rng, 7, b.nG)
+    M = b.overlap(C1, C2)
+    want = b.volume * (C1.conj() @ C2.T)                              # M[a, b] = Omega sum_n conj(C1[a,n]) C2[b,n]
+    assert M.shape == (4, 7) and np.max(np.abs(M - want)) <= 1e-13 * np.max(np.abs(want))
+    assert abs(b.overlap_entry(C1, C2, 3, 5) - want[3, 5]) <= 1e-13 * abs(want[3, 5])
+    assert np.allclose(b.overlap(C2, C1), M.conj().T, rtol=1e-14)
+
+
+# ------------------------------------------------------------------------------------------ Vnl
+
+def test_Vnl_dense_matrix_rank1_zeroD_denseD(ref):
+    cfg = 101
+    R, kpts, Ecut, S = workloads.lattice(cfg)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    assert b.nG <= 400
+    inp = workloads.make_inputs(cfg, b.iG)
+    P, D, C = inp["P"], inp["D"], inp["C"]
+    Pm = P.T                                        # nG x np
+    Vnl = Pm @ np.diag(D) @ Pm.conj().T             # dense nG x nG
+    want = C @ Vnl.T                                 # row b: Vnl @ C[b]
+    got = b.apply_Vnl(P, D, C)
+    assert np.max(np.abs(got - want)) <= 1e-13 * np.max(np.abs(want))
+    # projection alone
+    assert np.allclose(b.project(P, C), C @ Pm.conj(), rtol=1e-13, atol=1e-15)
+    # rank one: d p (p^+ c)
+    p, d = P[:1], np.array([0.7])
+    got = b.apply_Vnl(p, d, C)
+    want = np.stack([d[0] * p[0] * np.vdot(p[0], c) for c in C])
+    assert np.max(np.abs(got - want)) <= 1e-13 * np.max(np.abs(want))
+    # D = 0 => 0 ; accumulate adds
+    assert np.all(b.apply_Vnl(P, np.zeros_like(D), C) == 0)
+    base = np.ones_like(C)
+    assert np.allclose(b.apply_Vnl(P, D, C, out=base), 1.0 + b.apply_Vnl(P, D, C), rtol=1e-14)
+    # dense Hermitian D
+    rng = np.random.default_rng(4)
+    A = _rand_c(rng, P.shape[0], P.shape[0]); Dd = A + A.conj().T
+    got = b.apply_Vnl(P, Dd, C)
+    want = C @ (Pm @ Dd @ Pm.conj().T).T
+    assert np.max(np.abs(got - want)) <= 1e-12 * np.max(np.abs(want))
+
+
+# ------------------------------------------------------------------------------------------ H
+
+def test_plane_wave_eigenvalue(ref):
+    """C = e_n, V_loc = (Omega/N) V0, no projectors => HC = (ke[n] + V0) Omega e_n, zero elsewhere."""
+    R, kpts, Ecut, S = workloads.lattice(101)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    V0 = -0.37
+    V = np.full(b.shape, V0 * b.volume / b.N)
+    for n0 in (0, 17, b.nG - 1):
+        C = np.zeros((1, b.nG), complex); C[0, n0] = 1.0 - 0.5j
+        HC = b.apply_H(V, None, None, C)[0]
+        want = np.zeros(b.nG, complex); want[n0] = (b.ke[n0] + V0) * b.volume * C[0, n0]
+        assert np.max(np.abs(HC - want)) <= 1e-13 * b.volume
+        ray = np.vdot(C[0], HC) / np.vdot(C[0], b.apply_O(C)[0])
+        assert abs(ray - (b.ke[n0] + V0)) <= 1e-13
+
+
+def test_H_is_sum_of_its_terms_and_hermitian(ref):
+    cfg = 102
+    R, kpts, Ecut, S = workloads.lattice(cfg)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    inp = workloads.make_inputs(cfg, b.iG, nb=4)
+    V, P, D, C = inp["Vloc"], inp["P"], inp["D"], inp["C"]
+    HC = b.apply_H(V, P, D, C)
+    terms = -0.5 * b.apply_L(C) + b.apply_Idag(V[None] * b.apply_I(C)) + b.apply_Vnl(P, D, C)
+    assert np.max(np.abs(HC - terms)) <= 1e-13 * np.max(np.abs(HC))
+    # Hermiticity to 1e-12 (north_star): a^+ H b = conj(b^+ H a)
+    rng = np.random.default_rng(8)
+    ab = _rand_c(rng, 2, b.nG)
+    Hab = b.apply_H(V, P, D, ab)
+    lhs, rhs = np.vdot(ab[0], Hab[1]), np.conj(np.vdot(ab[1], Hab[0]))
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(ab[0]) * np.linalg.norm(Hab[1])
+    # and with a dense Hermitian D
+    A = _rand_c(rng, P.shape[0], P.shape[0]); Dd = A + A.conj().T
+    Hab = b.apply_H(V, P, Dd, ab)
+    lhs, rhs = np.vdot(ab[0], Hab[1]), np.conj(np.vdot(ab[1], Hab[0]))
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(ab[0]) * np.linalg.norm(Hab[1])
+
+
+def test_translation_covariance(ref):
+    """Roll V_loc by grid vector s, move atoms by s/S, C'_m = exp(-2 pi i m.s/S) C_m
+    => (H'C')_m = exp(-2 pi i m.s/S) (HC)_m.  Pins the FFT sign against the structure-factor sign."""
+    cfg = 105
+    R, kpts, Ecut, S = workloads.lattice(cfg)
+    k = kpts[0]
+    b = ref.RefBasis(R, k, Ecut, S)
+    atoms = workloads.atoms_fractional(cfg)
+    V = workloads.make_vloc(cfg, atoms)
+    D = workloads.make_D(cfg)
+    C = workloads.make_bands(cfg, b.nG, nb=3)
+    P = workloads.make_projectors(cfg, b.iG, k, atoms)
+    HC = b.apply_H(V, P, D, C)
+    s = np.array([3, -4, 5])
+    atoms2 = atoms + s / np.asarray(S, dtype=float)
+    V2 = np.roll(V, shift=tuple(s), axis=(0, 1, 2))
+    P2 = workloads.make_projectors(cfg, b.iG, k, atoms2)
+    ph = np.exp(-2j * np.pi * (b.iG * (s / np.asarray(S, dtype=float))).sum(1))
+    # projectors carry exp(-2 pi i (m + k).x): the k part is a global phase per atom and cancels in P D P^+
+    HC2 = b.apply_H(V2, P2, D, C * ph[None, :])
+    assert np.max(np.abs(HC2 - ph[None, :] * HC)) <= 1e-12 * np.max(np.abs(HC))

@@ -1,0 +1,41 @@
+"""Workload table mirroring BASELINE.json:configs[0..4] (ids 1..5) plus small test-only shapes.
+
+Fields: cell (orthorhombic edge lengths, bohr), kpoints (reduced), Ecut (Ha), S (FFT box), nb (bands
+per k), natoms, n_lm (projectors per atom: 4 = s,p ; 9 = s,p,d), atoms (placement rule), extra
+(additional term in V).  Exact nG per (config, k) is in tests/golden/basis_counts.txt.
+"""
+
+CONFIGS = {
+    1: dict(name="cfg1_cubic10_G_32^3", cell=(10.0, 10.0, 10.0), kpoints=[(0.0, 0.0, 0.0)], Ecut=10.0,
+            S=(32, 32, 32), nb=8, natoms=2, n_lm=4, atoms="uniform", extra="noise"),
+    2: dict(name="cfg2_cubic20.5_k.25_80^3", cell=(20.5, 20.5, 20.5), kpoints=[(0.25, 0.25, 0.25)], Ecut=15.0,
+            S=(80, 80, 80), nb=128, natoms=64, n_lm=4, atoms="uniform", extra=None),
+    3: dict(name="cfg3_molbox30_G_128^3", cell=(30.0, 30.0, 30.0), kpoints=[(0.0, 0.0, 0.0)], Ecut=20.0,
+            S=(128, 128, 128), nb=256, natoms=32, n_lm=9, atoms="clustered", extra="cavity"),
+    4: dict(name="cfg4_slab20x20x60_4k_72x72x216", cell=(20.0, 20.0, 60.0),
+            kpoints=[(0.0, 0.0, 0.0), (0.5, 0.0, 0.0), (0.0, 0.5, 0.0), (0.5, 0.5, 0.0)], Ecut=15.0,
+            S=(72, 72, 216), nb=384, natoms=96, n_lm=4, atoms="slab", extra="ramp"),
+    5: dict(name="cfg5_bulk216_G_128^3", cell=(30.7, 30.7, 30.7), kpoints=[(0.0, 0.0, 0.0)], Ecut=20.0,
+            S=(128, 128, 128), nb=512, natoms=216, n_lm=4, atoms="lattice6", extra=None),
+}
+
+# Small shapes for parity tests: every radix (2, 3, 5) and mixed lengths, non-cubic boxes, k != 0,
+# sizes that span several tiles of the CUDA kernels and leave ragged tails.
+TEST_CONFIGS = {
+    101: dict(name="t_12x15x20", cell=(6.0, 7.5, 9.0), kpoints=[(0.1, -0.2, 0.3)], Ecut=4.0,
+              S=(12, 15, 20), nb=5, natoms=2, n_lm=4, atoms="uniform", extra="noise"),
+    102: dict(name="t_30x36x40", cell=(9.0, 11.0, 12.5), kpoints=[(0.25, 0.0, -0.4)], Ecut=8.0,
+              S=(30, 36, 40), nb=19, natoms=5, n_lm=9, atoms="uniform", extra="noise"),
+    103: dict(name="t_48x45x50", cell=(14.0, 13.0, 15.0), kpoints=[(0.0, 0.0, 0.0), (0.5, 0.5, 0.5)], Ecut=9.0,
+              S=(48, 45, 50), nb=37, natoms=11, n_lm=4, atoms="uniform", extra="ramp"),
+    104: dict(name="t_64^3", cell=(16.0, 16.0, 16.0), kpoints=[(0.0, 0.0, 0.0)], Ecut=12.0,
+              S=(64, 64, 64), nb=33, natoms=17, n_lm=4, atoms="lattice6", extra=None),
+    105: dict(name="t_27x25x32", cell=(8.0, 7.0, 9.5), kpoints=[(0.3, 0.3, 0.1)], Ecut=7.0,
+              S=(27, 25, 32), nb=9, natoms=3, n_lm=9, atoms="clustered", extra="cavity"),
+}
+
+
+def get_config(cfg_id):
+    if cfg_id in CONFIGS:
+        return CONFIGS[cfg_id]
+    return TEST_CONFIGS[cfg_id]

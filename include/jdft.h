@@ -1,0 +1,130 @@
+/*
+ * jdft.h -- C ABI of libjdft_b200: the data-parallel hot path of plane-wave DFT in the DFT++
+ * operator language used by JDFTx (arXiv 1708.03621), hand-written for NVIDIA B200 (sm_100a).
+ *
+ *     H C = -1/2 L C + I^+ Diag(V_loc) I C + P D P^+ C        (BASELINE.json north_star)
+ *
+ * What the paper fixes.  PAPER.md:76 (section 2.1): "the operators I and J Fourier transform from
+ * reciprocal to real space and vice versa (using Fast Fourier Transforms)"; gradient/divergence "apply in
+ * reciprocal space (where they are diagonal)"; integrals are "a dot product with the overlap operator O",
+ * which is "diagonal in the plane-wave basis".  PAPER.md:86: wavefunctions live in a ColumnBundle, the
+ * grid and its Fourier transforms in GridInfo.  PAPER.md:127: SpeciesInfo holds the pseudopotentials
+ * (the nonlocal projectors P and couplings D here).  PAPER.md:59 delegates every formula to the DFT++
+ * paper (its Ref. [11]); the concrete conventions below are the readings listed in DESIGN.md section 3.
+ *
+ * Conventions.
+ *   complex128  = double[2], (re, im) interleaved.
+ *   R           = 3x3 row-major, COLUMNS are the lattice vectors (bohr).  Omega = |det R|.
+ *   G           = 2 pi R^-1 (rows are reciprocal vectors); ke(m) = 1/2 (m+k)^T G G^T (m+k), k reduced.
+ *   basis       = { m in Z^3 : ke(m) < Ecut } in ascending signed lexicographic order of (m0, m1, m2),
+ *                 m2 fastest;  index[n] = ((m0 mod S0) S1 + (m1 mod S1)) S2 + (m2 mod S2).
+ *   C           = [nb][nG] band-major, G-sphere index contiguous.
+ *   psi         = [nb][S0][S1][S2] real-space block, axis 2 contiguous.
+ *   I           (I C)[j]   = sum_n C[n] exp(+2 pi i sum_d iG[n]_d j_d / S_d)      (unnormalised)
+ *   Idag        (I^+ f)[n] = sum_j exp(-2 pi i sum_d iG[n]_d j_d / S_d) f[j]
+ *   J           = I^+ / N,   N = S0 S1 S2          (J I = 1 on the sphere)
+ *   O C         = Omega C;   L C = -Omega |G+k|^2 C = -2 Omega ke C
+ *   Vnl         = P D P^+ with P = [np][nG] (projector-major) and D given as data
+ *
+ * Pointers.  Unless marked HOST, every data pointer is a DEVICE pointer on the basis' device, owned by
+ * the caller (e.g. a torch tensor's data_ptr()), 16-byte aligned.  The library owns only the basis
+ * object.  The hot path allocates nothing and never synchronises with the host: all scratch comes from
+ * the caller-supplied workspace, and kernels are enqueued on the caller's stream.  Input and output
+ * arrays must not alias unless stated.
+ *
+ * Errors.  Every call returns JDFT_OK (0) or a negative code; nothing throws, aborts or prints.
+ * jdft_last_error() returns a thread-local message for the last failure.  Launches are asynchronous:
+ * launch-time CUDA errors are returned, execution-time errors surface at the caller's next sync.
+ *
+ * The jdft_*_host entry points are the same operations taking HOST arrays: they allocate device
+ * buffers, copy in, run the same kernels, copy out and synchronise (used for the end-to-end number).
+ */
+#ifndef JDFT_H
+#define JDFT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define JDFT_OK 0
+#define JDFT_EINVAL (-1)     /* null pointer, negative size, bad mode, singular R                      */
+#define JDFT_EBOX (-2)       /* S[d] not 2^a 3^b 5^c, or box too small: two sphere points would collide */
+#define JDFT_EWORKSPACE (-3) /* no workspace set, or too small for one band                             */
+#define JDFT_ECUDA (-4)      /* a CUDA runtime call failed (see jdft_last_error)                        */
+#define JDFT_ENOMEM (-5)     /* host or device allocation failed (basis creation / *_host calls only)   */
+
+typedef struct jdft_basis jdft_basis; /* opaque; owned by the library */
+typedef void *jdft_stream;            /* a cudaStream_t; NULL = the legacy default stream */
+
+/* ---- basis (readings 6-12) --------------------------------------
+ * Builds the G-sphere of the wavefunction cutoff inside FFT box S, uploads the index map, ke = 1/2|G+k|^2,
+ * the per-axis twiddle tables and the column/plane structure used to prune the FFT passes.
+ * R, k, S are HOST arrays.  Fails with JDFT_EBOX when max(m_d) - min(m_d) >= S[d] for some axis.      */
+int jdft_basis_create(const double R[9], const double k[3], double Ecut, const int S[3], int device,
+                      jdft_basis **out);
+int jdft_basis_destroy(jdft_basis *b);
+/* sizes: nG plane waves, N = S0 S1 S2 grid points, cell volume Omega (any pointer may be NULL)        */
+int jdft_basis_info(const jdft_basis *b, int64_t *nG, int64_t *N, double *volume);
+/* pruning structure: occupied i0 planes and (i0,i1) columns (npl, ncol)               */
+int jdft_basis_structure(const jdft_basis *b, int64_t *npl, int64_t *ncol);
+/* HOST copies for bit-exact checks: iG int32[nG][3], index int32[nG], ke f64[nG] (any may be NULL)    */
+int jdft_basis_export(const jdft_basis *b, int32_t *iG_host, int32_t *index_host, double *ke_host);
+/* device pointers to the resident index map / ke (valid until destroy)                                 */
+int jdft_basis_device_maps(const jdft_basis *b, const int32_t **index_dev, const double **ke_dev);
+
+/* ---- workspace -------------------------------------------------------------------------------------
+ * Bytes needed to process `nbands_batch` bands at once (FFT intermediates) and to run the projector /
+ * overlap GEMMs with up to `nrows_max` rows (max of nproj, nb) -- the two phases share the buffer.
+ * Calls with more bands than fit are split into band batches internally (results are identical).      */
+size_t jdft_workspace_bytes(const jdft_basis *b, int nbands_batch, int nrows_max);
+int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
+/* tunables: "band_batch" (bands per FFT batch, 0 = automatic), "force_generic_fft" (0/1: use the
+ * runtime-radix FFT kernels even for lengths that have specialised ones; for tests)                   */
+int jdft_set_option(jdft_basis *b, const char *key, int64_t value);
+
+/* ---- operators ------------------------------------------------------ */
+/* I: C [nb][nG] -> psi [nb][N]   (scatter + inverse 3-D FFT, unnormalised, sign +)                    */
+int jdft_apply_I(const jdft_basis *b, const double *C, int nb, double *psi, jdft_stream s);
+/* Idag: psi [nb][N] -> C [nb][nG] (forward 3-D FFT, sign -, + gather)                                 */
+int jdft_apply_Idag(const jdft_basis *b, const double *psi, int nb, double *C, jdft_stream s);
+/* J = Idag / N                                                                                        */
+int jdft_apply_J(const jdft_basis *b, const double *psi, int nb, double *C, jdft_stream s);
+/* L C = -2 Omega ke C ; O C = Omega C.  May run in place (out == C).                                  */
+int jdft_apply_L(const jdft_basis *b, const double *C, int nb, double *LC, jdft_stream s);
+int jdft_apply_O(const jdft_basis *b, const double *C, int nb, double *OC, jdft_stream s);
+/* Vnl: out (+)= P D P^+ C.  P c128[nproj][nG]; D_mode 0: D = f64[nproj] real diagonal;
+ * D_mode 1: D = c128[nproj][nproj] row-major Hermitian; accumulate != 0 adds into out.               */
+int jdft_apply_Vnl(const jdft_basis *b, const double *P, int nproj, const double *D, int D_mode,
+                   const double *C, int nb, double *out, int accumulate, jdft_stream s);
+/* projection alone: Bproj [nb][nproj] = (P^+ C)^T, i.e. Bproj[ib][j] = sum_n conj(P[j][n]) C[ib][n]   */
+int jdft_project(const jdft_basis *b, const double *P, int nproj, const double *C, int nb, double *Bproj,
+                 jdft_stream s);
+/* H: HC = -1/2 L C + I^+ (Vloc .* I C) + P D P^+ C.  Vloc f64[N] is used exactly as passed (the caller
+ * folds in the quadrature weight Omega/N; reading 5).  nproj == 0 skips the nonlocal term.  */
+int jdft_apply_H(const jdft_basis *b, const double *Vloc, const double *P, int nproj, const double *D,
+                 int D_mode, const double *C, int nb, double *HC, jdft_stream s);
+/* overlap: M[a + nb1*bb] = Omega sum_n conj(C1[a][n]) C2[bb][n]  (column-major nb1 x nb2, c128)       */
+int jdft_overlap(const jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M,
+                 jdft_stream s);
+
+/* ---- HOST-buffer variants (end-to-end path: H2D copy, kernels, D2H copy, sync) -------------------- */
+int jdft_apply_H_host(jdft_basis *b, const double *Vloc_host, const double *P_host, int nproj,
+                      const double *D_host, int D_mode, const double *C_host, int nb, double *HC_host);
+int jdft_overlap_host(jdft_basis *b, const double *C1_host, int nb1, const double *C2_host, int nb2,
+                      double *M_host);
+
+/* ---- diagnostics ---------------------------------------------------------------------------------- */
+const char *jdft_last_error(void);
+/* kernels launched by this thread since the last call with reset != 0 (bench.py's gpu_launches)       */
+int64_t jdft_launch_count(int reset);
+/* per-kernel-group device time of the LAST apply_H / overlap call when "profile" option is on:
+ * not part of the hot path.                                                                           */
+const char *jdft_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JDFT_H */

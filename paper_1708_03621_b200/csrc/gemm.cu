@@ -1,0 +1,290 @@
+// Complex FP64 GEMMs on the FP64 tensor pipe (DMMA, mma.sync.m8n8k4.f64) for the nonlocal projectors and the
+// subspace overlap.  tcgen05 has no FP64 kind, so on sm_100a the FP64 tensor path is
+// the warp-level DMMA; one complex MAC tile = four real DMMAs (Cr += ArBr -/+ AiBi, Ci += ArBi +/- AiBr).
+//
+//   k_gemm_dotk   Out[r][c] = sum_k X[r][k] * conj?(Y[c][k])     both operands K-contiguous (K = nG), split-K with
+//                 a fixed-order reduction (deterministic, no atomics): P^+ C, C1^+ C2, and D.B for dense D
+//   k_gemm_expand Out[r][n] (+)= sum_j A[r][j] * Pm[j][n]        K = nproj, n contiguous: P (D P^+ C)
+//
+// Tiles: 64 x 64 per CTA, 4 warps of 32 x 32 (4 x 4 DMMA tiles of 8 x 8), BK = 8, 4-stage cp.async pipeline.
+// Shared-memory layout of a K-contiguous operand: per group of 4 k, a dense [64 rows][4 k] block of c128
+// (64 B per row, so the 8 lanes of a quarter-warp read 128 contiguous bytes), blocks skewed by 64 B.
+#include "jdft_internal.h"
+
+namespace {
+
+constexpr int BM = 64, BN = 64, BK = 8, STAGES = 4, NTHREADS = 128;
+constexpr int KBLK_BYTES = 64 * 64 + 64;               // one [64][4] block + skew
+constexpr int OPK_BYTES = (BK / 4) * KBLK_BYTES;        // K-contiguous operand, one stage
+constexpr int PROW_BYTES = BN * 16 + 32;                // n-contiguous operand: row stride
+constexpr int OPN_BYTES = BK * PROW_BYTES;
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool valid) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    const int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma(double &c0, double &c1, const double a, const double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// load one stage of a K-contiguous operand: rows [row0, row0+64) of M [nrows][ld], k in [k0, k0+BK), zero beyond kend/nrows
+__device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld, int nrows, int row0, int64_t k0,
+                                         int64_t kend, int tid) {
+#pragma unroll
+    for (int i = 0; i < (64 * BK) / NTHREADS; i++) {
+        const int e = tid + i * NTHREADS;
+        const int r = e / BK, kk = e % BK;
+        const int64_t k = k0 + kk;
+        const bool ok = (row0 + r < nrows) && (k < kend);
+        const double2 *src = ok ? M + (size_t)(row0 + r) * ld + k : M;
+        cp_async16(dst + (kk / 4) * KBLK_BYTES + r * 64 + (kk % 4) * 16, src, ok);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------- dot-K GEMM
+template <bool CONJY>
+__global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
+                                                        const double2 *__restrict__ Y, const int Cn, const int64_t K,
+                                                        const int ktiles_per_split, double2 *__restrict__ part) {
+    extern __shared__ __align__(16) char smem[];
+    char *sX = smem, *sY = smem + STAGES * OPK_BYTES;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wr = (warp >> 1) * 32, wc = (warp & 1) * 32;
+    const int row0 = blockIdx.y * BM, col0 = blockIdx.x * BN;
+    const int64_t ktiles = (K + BK - 1) / BK;
+    const int64_t kt0 = (int64_t)blockIdx.z * ktiles_per_split;
+    int64_t kt1 = kt0 + ktiles_per_split;
+    if (kt1 > ktiles) kt1 = ktiles;
+    const int nkt = (int)(kt1 - kt0);
+
+    double cr[4][4][2], ci[4][4][2];
+#pragma unroll
+    for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < 4; j++) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+
+    for (int s = 0; s < STAGES - 1; s++) {
+        if (s < nkt) {
+            load_opk(sX + s * OPK_BYTES, X, K, Rn, row0, (kt0 + s) * BK, K, tid);
+            load_opk(sY + s * OPK_BYTES, Y, K, Cn, col0, (kt0 + s) * BK, K, tid);
+        }
+        cp_async_commit();
+    }
+    const int fo = (lane >> 2) * 64 + (lane & 3) * 16;  // fragment offset inside a [64][4] block
+    for (int kt = 0; kt < nkt; kt++) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            const int nx = kt + STAGES - 1;
+            if (nx < nkt) {
+                const int slot = nx % STAGES;
+                load_opk(sX + slot * OPK_BYTES, X, K, Rn, row0, (kt0 + nx) * BK, K, tid);
+                load_opk(sY + slot * OPK_BYTES, Y, K, Cn, col0, (kt0 + nx) * BK, K, tid);
+            }
+            cp_async_commit();
+        }
+        const char *bx = sX + (kt % STAGES) * OPK_BYTES, *by = sY + (kt % STAGES) * OPK_BYTES;
+#pragma unroll
+        for (int kk = 0; kk < BK / 4; kk++) {
+            double2 a[4], bq[4];
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+                a[i] = *reinterpret_cast<const double2 *>(bx + kk * KBLK_BYTES + (wr + 8 * i) * 64 + fo);
+#pragma unroll
+            for (int j = 0; j < 4; j++)
+                bq[j] = *reinterpret_cast<const double2 *>(by + kk * KBLK_BYTES + (wc + 8 * j) * 64 + fo);
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    // X (Yr -/+ i Yi):  conj: Cr += XrYr + XiYi, Ci += XiYr - XrYi ; else Cr += XrYr - XiYi, Ci += XiYr + XrYi
+                    const double yi = CONJY ? bq[j].y : -bq[j].y;
+                    dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
+                    dmma(ci[i][j][0], ci[i][j][1], a[i].y, bq[j].x);
+                    dmma(cr[i][j][0], cr[i][j][1], a[i].y, yi);
+                    dmma(ci[i][j][0], ci[i][j][1], a[i].x, -yi);
+                }
+        }
+    }
+    cp_async_wait<0>();
+    double2 *P = part + (size_t)blockIdx.z * Rn * Cn;
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        const int r = row0 + wr + 8 * i + (lane >> 2);
+        if (r >= Rn) continue;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            const int c = col0 + wc + 8 * j + 2 * (lane & 3);
+            if (c < Cn) P[(size_t)r * Cn + c] = make_double2(cr[i][j][0], ci[i][j][0]);
+            if (c + 1 < Cn) P[(size_t)r * Cn + c + 1] = make_double2(cr[i][j][1], ci[i][j][1]);
+        }
+    }
+}
+
+// Out[i] = scale * dscale[c] * sum_s part[s][i]   (fixed order)
+__global__ void k_splitk_reduce(const double2 *__restrict__ part, const int nsplit, const int64_t total, const int Cn,
+                                const double scale, const double *__restrict__ dscale, double2 *__restrict__ Out) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        double sr = 0.0, si = 0.0;
+        for (int s = 0; s < nsplit; s++) {
+            const double2 v = part[(size_t)s * total + i];
+            sr += v.x;
+            si += v.y;
+        }
+        const double f = dscale ? scale * dscale[i % Cn] : scale;
+        Out[i] = make_double2(f * sr, f * si);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------- expand GEMM
+__global__ void __launch_bounds__(NTHREADS) k_gemm_expand(const double2 *__restrict__ A, const int Rn,
+                                                          const double2 *__restrict__ Pm, const int K, const int64_t Nn,
+                                                          double2 *__restrict__ Out, const int accumulate) {
+    extern __shared__ __align__(16) char smem[];
+    char *sA = smem, *sP = smem + STAGES * OPK_BYTES;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wr = (warp >> 1) * 32, wc = (warp & 1) * 32;
+    const int row0 = blockIdx.y * BM;
+    const int64_t n0 = (int64_t)blockIdx.x * BN;
+    const int nkt = (K + BK - 1) / BK;
+
+    double cr[4][4][2], ci[4][4][2];
+#pragma unroll
+    for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < 4; j++) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+
+    auto load_p = [&](char *dst, int k0) {
+#pragma unroll
+        for (int i = 0; i < (BK * BN) / NTHREADS; i++) {
+            const int e = tid + i * NTHREADS;
+            const int kk = e / BN, nn = e % BN;
+            const bool ok = (k0 + kk < K) && (n0 + nn < Nn);
+            const double2 *src = ok ? Pm + (size_t)(k0 + kk) * Nn + n0 + nn : Pm;
+            cp_async16(dst + kk * PROW_BYTES + nn * 16, src, ok);
+        }
+    };
+    for (int s = 0; s < STAGES - 1; s++) {
+        if (s < nkt) {
+            load_opk(sA + s * OPK_BYTES, A, K, Rn, row0, (int64_t)s * BK, K, tid);
+            load_p(sP + s * OPN_BYTES, s * BK);
+        }
+        cp_async_commit();
+    }
+    const int fa = (lane >> 2) * 64 + (lane & 3) * 16;
+    const int fp = (lane & 3) * PROW_BYTES + (lane >> 2) * 16;
+    for (int kt = 0; kt < nkt; kt++) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            const int nx = kt + STAGES - 1;
+            if (nx < nkt) {
+                const int slot = nx % STAGES;
+                load_opk(sA + slot * OPK_BYTES, A, K, Rn, row0, (int64_t)nx * BK, K, tid);
+                load_p(sP + slot * OPN_BYTES, nx * BK);
+            }
+            cp_async_commit();
+        }
+        const char *ba = sA + (kt % STAGES) * OPK_BYTES, *bp = sP + (kt % STAGES) * OPN_BYTES;
+#pragma unroll
+        for (int kk = 0; kk < BK / 4; kk++) {
+            double2 a[4], bq[4];
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+                a[i] = *reinterpret_cast<const double2 *>(ba + kk * KBLK_BYTES + (wr + 8 * i) * 64 + fa);
+#pragma unroll
+            for (int j = 0; j < 4; j++)
+                bq[j] = *reinterpret_cast<const double2 *>(bp + kk * 4 * PROW_BYTES + (wc + 8 * j) * 16 + fp);
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
+                    dmma(ci[i][j][0], ci[i][j][1], a[i].y, bq[j].x);
+                    dmma(cr[i][j][0], cr[i][j][1], a[i].y, -bq[j].y);
+                    dmma(ci[i][j][0], ci[i][j][1], a[i].x, bq[j].y);
+                }
+        }
+    }
+    cp_async_wait<0>();
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        const int r = row0 + wr + 8 * i + (lane >> 2);
+        if (r >= Rn) continue;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            const int64_t n = n0 + wc + 8 * j + 2 * (lane & 3);
+            double2 *o = Out + (size_t)r * Nn + n;
+            if (n < Nn) {
+                double2 v = make_double2(cr[i][j][0], ci[i][j][0]);
+                if (accumulate) { const double2 w = o[0]; v.x += w.x; v.y += w.y; }
+                o[0] = v;
+            }
+            if (n + 1 < Nn) {
+                double2 v = make_double2(cr[i][j][1], ci[i][j][1]);
+                if (accumulate) { const double2 w = o[1]; v.x += w.x; v.y += w.y; }
+                o[1] = v;
+            }
+        }
+    }
+}
+
+template <class K>
+cudaError_t ensure_smem(K kernel, size_t bytes) {
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+}  // namespace
+
+int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y, int Cn, int64_t K, int conjY,
+                   double scale, const double *dscale, double *Out, void *scratch, size_t scratch_bytes,
+                   cudaStream_t st) {
+    (void)b;
+    if (Rn <= 0 || Cn <= 0) return JDFT_OK;
+    const int64_t ktiles = (K + BK - 1) / BK;
+    const int tiles = ((Rn + BM - 1) / BM) * ((Cn + BN - 1) / BN);
+    const size_t one = (size_t)Rn * Cn * 16;
+    int64_t nsplit = (148 * 3 + tiles - 1) / tiles;
+    if (nsplit > ktiles / 8) nsplit = ktiles / 8;
+    if (nsplit < 1) nsplit = 1;
+    if ((size_t)nsplit * one > scratch_bytes) nsplit = (int64_t)(scratch_bytes / one);
+    if (nsplit < 1) return jdft_fail(JDFT_EWORKSPACE, "gemm: workspace too small for a %d x %d result", Rn, Cn);
+    int64_t per = (ktiles + nsplit - 1) / nsplit;
+    if (per < 1) per = 1;
+    nsplit = (ktiles + per - 1) / per;
+    if (nsplit < 1) nsplit = 1;
+    const size_t smem = 2 * STAGES * OPK_BYTES;
+    dim3 grid((Cn + BN - 1) / BN, (Rn + BM - 1) / BM, (unsigned)nsplit);
+    if (conjY) {
+        JDFT_CUDA(ensure_smem(k_gemm_dotk<true>, smem));
+        k_gemm_dotk<true><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
+    } else {
+        JDFT_CUDA(ensure_smem(k_gemm_dotk<false>, smem));
+        k_gemm_dotk<false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
+    }
+    JDFT_LAUNCH_CHECK("k_gemm_dotk");
+    const int64_t total = (int64_t)Rn * Cn;
+    int64_t blocks = (total + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, total, Cn, scale, dscale, (double2 *)Out);
+    JDFT_LAUNCH_CHECK("k_splitk_reduce");
+    return JDFT_OK;
+}
+
+int jdft_gemm_expand(const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
+                     cudaStream_t st) {
+    if (Rn <= 0 || Nn <= 0) return JDFT_OK;
+    const size_t smem = STAGES * (OPK_BYTES + OPN_BYTES);
+    JDFT_CUDA(ensure_smem(k_gemm_expand, smem));
+    dim3 grid((unsigned)((Nn + BN - 1) / BN), (Rn + BM - 1) / BM);
+    k_gemm_expand<<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, accumulate);
+    JDFT_LAUNCH_CHECK("k_gemm_expand");
+    return JDFT_OK;
+}

@@ -1,0 +1,80 @@
+// Internal declarations shared by the translation units of libjdft_b200 (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <vector>
+#include "../../include/jdft.h"
+
+#define JDFT_MAX_PASSES 12
+
+// Radix plan of one 1-D FFT length (Stockham autosort, one radix per pass).
+struct FftPlan {
+    int L;
+    int npass;
+    int radix[JDFT_MAX_PASSES];
+};
+
+struct jdft_basis {
+    // geometry
+    double R[9], k[3], Ecut, G[9], GGT[9], volume;
+    int S[3];
+    int64_t N, nG;
+    int device;
+    // host copies of the sphere
+    std::vector<int32_t> iG, index;
+    std::vector<double> ke;
+    // pruning structure: planes p <-> m0 = m0lo + p; columns c of plane p <-> m1 = pl_m1lo[p] + (c - pl_cbase[p])
+    int npl, m0lo, ncol, maxcol_per_plane;
+    std::vector<int> pl_m1lo, pl_cbase;       // [npl], [npl+1]
+    std::vector<int> col_n0, col_m2lo;        // [ncol+1], [ncol]
+    // device copies
+    int32_t *d_index;
+    double *d_ke;
+    int *d_col_n0, *d_col_m2lo;               // [ncol+1], [ncol]
+    int *d_rowcol;                            // [npl][S1]: column index of (plane p, i1) or -1
+    int *d_planeof;                           // [S0]: plane index of i0 or -1
+    double2 *d_tw[3];                         // exp(+2 pi i t / S_d), t = 0..S_d-1
+    FftPlan plan[3];
+    // workspace (caller-owned)
+    void *ws;
+    size_t ws_bytes;
+    // options
+    int64_t opt_band_batch, opt_force_generic;
+    // cached device buffers of the *_host entry points (library-owned, grow-only)
+    void *hb[8];
+    size_t hb_bytes[8];
+};
+
+// error plumbing
+int jdft_fail(int code, const char *fmt, ...);
+int jdft_cuda_fail(cudaError_t e, const char *what);
+void jdft_count_launch(int n);
+#define JDFT_CUDA(call)                                           \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return jdft_cuda_fail(e__, #call); \
+    } while (0)
+#define JDFT_LAUNCH_CHECK(name)                                   \
+    do {                                                          \
+        jdft_count_launch(1);                                     \
+        cudaError_t e__ = cudaGetLastError();                     \
+        if (e__ != cudaSuccess) return jdft_cuda_fail(e__, name); \
+    } while (0)
+
+// per-band scratch of the FFT path (bytes)
+size_t jdft_fft_bytes_per_band(const jdft_basis *b);
+// bands per batch given the workspace and options; 0 if not even one fits
+int jdft_band_batch(const jdft_basis *b, int nb);
+
+// local.cu: FFT-based pieces
+int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C, int nb, double *HC, cudaStream_t st);
+
+// gemm.cu
+// Out[r][c] = scale * dscale[c] * sum_k X[r][k] * (conjY ? conj(Y[c][k]) : Y[c][k]);  X [Rn][K], Y [Cn][K], Out [Rn][Cn]
+int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y, int Cn, int64_t K, int conjY,
+                   double scale, const double *dscale, double *Out, void *scratch, size_t scratch_bytes,
+                   cudaStream_t st);
+// Out[r][n] (+)= sum_j A[r][j] * Pm[j][n];  A [Rn][K] (K contiguous), Pm [K][Nn] (n contiguous), Out [Rn][Nn]
+int jdft_gemm_expand(const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
+                     cudaStream_t st);

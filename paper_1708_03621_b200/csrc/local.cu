@@ -1,0 +1,394 @@
+// FFT-based operators: I, I^+, J, the local + kinetic part of H, and the diagonal L, O.
+// Pipeline of one band batch of apply_H (SURVEY.md 3.3 / DESIGN.md section 5):
+//   K1 k_cols_inv   scatter sphere -> columns  (+) inverse FFT along axis 2   (occupied (i0,i1) columns only)
+//   K2 k_rows<inv>  inverse FFT along axis 1, compact columns -> dense planes  (occupied i0 planes only)
+//   K3 k_planes<V>  inverse FFT along axis 0 (+) * V_loc (+) forward FFT along axis 0 (real-space psi never stored)
+//   K4 k_rows<fwd>  forward FFT along axis 1, dense planes -> compact columns
+//   K5 k_cols_fwd   forward FFT along axis 2 (+) gather box -> sphere (+) + Omega ke C   (the -1/2 L C term)
+// Intermediates: W1 [nbatch][ncol][S2] and W2 [nbatch][npl][S1][S2] (c128) in the caller's workspace.
+#include "fft.cuh"
+
+using namespace jfft;
+
+namespace {
+
+constexpr int kT = 8;      // pencils per CTA
+constexpr int kNT = 128;   // threads per CTA
+
+__device__ __forceinline__ int wrapi(int m, int S) {
+    int r = m % S;
+    return r < 0 ? r + S : r;
+}
+
+// ------------------------------------------------------------------------------------------------ K1
+template <int LT>
+__global__ void __launch_bounds__(kNT) k_cols_inv(const FftPlan plan, const double2 *__restrict__ tw, const int ncol,
+                                                  const int64_t nG, const int *__restrict__ col_n0,
+                                                  const int *__restrict__ col_m2lo, const double2 *__restrict__ C,
+                                                  double2 *__restrict__ W1) {
+    constexpr int T = kT, TP = kT + 1, NT = kNT;
+    const int L = LT > 0 ? LT : plan.L;
+    extern __shared__ double2 smem[];
+    double2 *bufA = smem, *bufB = smem + L * TP;
+    __shared__ int s_n0[T + 1], s_m2[T];
+    const int tid = threadIdx.x, c0 = blockIdx.x * T, b = blockIdx.y;
+    const int nc = min(T, ncol - c0);
+    if (tid <= T) s_n0[tid] = col_n0[min(c0 + tid, ncol)];
+    if (tid < T) s_m2[tid] = col_m2lo[min(c0 + tid, ncol - 1)];
+    for (int e = tid; e < L * TP; e += NT) bufB[e] = make_double2(0.0, 0.0);
+    __syncthreads();
+    const int nbeg = s_n0[0], nend = s_n0[nc];
+    const double2 *Cb = C + (size_t)b * nG;
+    for (int e = tid; e < nend - nbeg; e += NT) {
+        const int n = nbeg + e;
+        int t = 0;
+        while (n >= s_n0[t + 1]) t++;
+        const int row = wrapi(s_m2[t] + (n - s_n0[t]), L);
+        bufB[row * TP + t] = Cb[n];
+    }
+    __syncthreads();
+    double2 *out = fft_out_buf(fft_npass<LT>(plan)) ? bufB : bufA;
+    fft_run<LT, +1, T, TP, NT>(
+        plan, tw, bufA, bufB, [&](int row, int t) { return bufB[row * TP + t]; },
+        [&](int row, int t, double2 v) { out[row * TP + t] = v; });
+    __syncthreads();
+    double2 *Wb = W1 + ((size_t)b * ncol + c0) * L;
+    for (int e = tid; e < nc * L; e += NT) {
+        const int t = e / L, row = e - t * L;
+        Wb[e] = out[row * TP + t];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K5
+// out[b][n] = scale * (F_2 W1)[column of n][m2 of n]  (+ kin * ke[n] * C[b][n])
+template <int LT>
+__global__ void __launch_bounds__(kNT) k_cols_fwd(const FftPlan plan, const double2 *__restrict__ tw, const int ncol,
+                                                  const int64_t nG, const int *__restrict__ col_n0,
+                                                  const int *__restrict__ col_m2lo, const double2 *__restrict__ W1,
+                                                  const double scale, const double kin, const double *__restrict__ ke,
+                                                  const double2 *__restrict__ C, double2 *__restrict__ outC) {
+    constexpr int T = kT, TP = kT + 1, NT = kNT;
+    const int L = LT > 0 ? LT : plan.L;
+    extern __shared__ double2 smem[];
+    double2 *bufA = smem, *bufB = smem + L * TP;
+    __shared__ int s_n0[T + 1], s_m2[T];
+    const int tid = threadIdx.x, c0 = blockIdx.x * T, b = blockIdx.y;
+    const int nc = min(T, ncol - c0);
+    if (tid <= T) s_n0[tid] = col_n0[min(c0 + tid, ncol)];
+    if (tid < T) s_m2[tid] = col_m2lo[min(c0 + tid, ncol - 1)];
+    const double2 *Wb = W1 + ((size_t)b * ncol + c0) * L;
+    for (int e = tid; e < T * L; e += NT) {
+        const int t = e / L, row = e - t * L;
+        bufB[row * TP + t] = t < nc ? Wb[e] : make_double2(0.0, 0.0);
+    }
+    __syncthreads();
+    double2 *out = fft_out_buf(fft_npass<LT>(plan)) ? bufB : bufA;
+    fft_run<LT, -1, T, TP, NT>(
+        plan, tw, bufA, bufB, [&](int row, int t) { return bufB[row * TP + t]; },
+        [&](int row, int t, double2 v) { out[row * TP + t] = v; });
+    __syncthreads();
+    const int nbeg = s_n0[0], nend = s_n0[nc];
+    const double2 *Cb = C + (size_t)b * nG;
+    double2 *Ob = outC + (size_t)b * nG;
+    for (int e = tid; e < nend - nbeg; e += NT) {
+        const int n = nbeg + e;
+        int t = 0;
+        while (n >= s_n0[t + 1]) t++;
+        const int row = wrapi(s_m2[t] + (n - s_n0[t]), L);
+        double2 v = out[row * TP + t];
+        v.x *= scale;
+        v.y *= scale;
+        if (kin != 0.0) {
+            const double f = kin * ke[n];
+            const double2 c = Cb[n];
+            v.x = fma(f, c.x, v.x);
+            v.y = fma(f, c.y, v.y);
+        }
+        Ob[n] = v;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K2 / K4
+// FWD == false: W1 columns -> (inverse FFT along axis 1) -> W2 planes.   FWD == true: the reverse, forward FFT.
+template <int LT, bool FWD>
+__global__ void __launch_bounds__(kNT) k_rows(const FftPlan plan, const double2 *__restrict__ tw, const int S2,
+                                              const int npl, const int ncol, const int *__restrict__ rowcol,
+                                              double2 *__restrict__ W1, double2 *__restrict__ W2) {
+    constexpr int T = kT, TP = kT, NT = kNT;
+    const int L = LT > 0 ? LT : plan.L;  // = S1
+    extern __shared__ double2 smem[];
+    double2 *bufA = smem, *bufB = smem + L * TP;
+    int *s_rowcol = reinterpret_cast<int *>(smem + 2 * L * TP);
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, p = blockIdx.y, b = blockIdx.z;
+    for (int i = tid; i < L; i += NT) s_rowcol[i] = rowcol[p * L + i];
+    __syncthreads();
+    double2 *W1b = W1 + (size_t)b * ncol * S2 + t0;
+    double2 *W2b = W2 + ((size_t)b * npl + p) * L * S2 + t0;
+    const int tmax = S2 - t0;
+    if (!FWD) {
+        fft_run<LT, +1, T, TP, NT>(
+            plan, tw, bufA, bufB,
+            [&](int row, int t) {
+                const int c = s_rowcol[row];
+                return (c >= 0 && t < tmax) ? W1b[(size_t)c * S2 + t] : make_double2(0.0, 0.0);
+            },
+            [&](int row, int t, double2 v) {
+                if (t < tmax) W2b[(size_t)row * S2 + t] = v;
+            });
+    } else {
+        fft_run<LT, -1, T, TP, NT>(
+            plan, tw, bufA, bufB,
+            [&](int row, int t) { return t < tmax ? W2b[(size_t)row * S2 + t] : make_double2(0.0, 0.0); },
+            [&](int row, int t, double2 v) {
+                const int c = s_rowcol[row];
+                if (c >= 0 && t < tmax) W1b[(size_t)c * S2 + t] = v;
+            });
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K3
+// MODE 0: W2 -> inverse axis 0 -> * V -> forward axis 0 -> W2 (in place; each CTA owns its pencils)
+// MODE 1: W2 -> inverse axis 0 -> psi (full box)          [last step of I]
+// MODE 2: psi (full box) -> forward axis 0 -> W2           [first step of I^+]
+template <int LT, int MODE>
+__global__ void __launch_bounds__(kNT) k_planes(const FftPlan plan, const double2 *__restrict__ tw, const int S1,
+                                                const int S2, const int npl, const int *__restrict__ planeof,
+                                                double2 *__restrict__ W2, const double *__restrict__ V,
+                                                double2 *__restrict__ psi) {
+    constexpr int T = kT, TP = kT, NT = kNT;
+    const int L = LT > 0 ? LT : plan.L;  // = S0
+    extern __shared__ double2 smem[];
+    double2 *bufA = smem, *bufB = smem + L * TP;
+    int *s_planeof = reinterpret_cast<int *>(smem + 2 * L * TP);
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y, b = blockIdx.z;
+    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    __syncthreads();
+    const size_t plane = (size_t)S1 * S2;
+    double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
+    const int tmax = S2 - t0;
+    auto ld_w2 = [&](int row, int t) {
+        const int p = s_planeof[row];
+        return (p >= 0 && t < tmax) ? W2b[p * plane + t] : make_double2(0.0, 0.0);
+    };
+    auto st_w2 = [&](int row, int t, double2 v) {
+        const int p = s_planeof[row];
+        if (p >= 0 && t < tmax) W2b[p * plane + t] = v;
+    };
+    if (MODE == 0) {
+        const int np = fft_npass<LT>(plan);
+        double2 *X = fft_out_buf(np) ? bufB : bufA;
+        double2 *Y = fft_out_buf(np) ? bufA : bufB;
+        const double *Vb = V + (size_t)i1 * S2 + t0;
+        fft_run<LT, +1, T, TP, NT>(plan, tw, bufA, bufB, ld_w2, [&](int row, int t, double2 v) {
+            const double f = t < tmax ? Vb[row * plane + t] : 0.0;
+            X[row * TP + t] = make_double2(v.x * f, v.y * f);
+        });
+        __syncthreads();
+        fft_run<LT, -1, T, TP, NT>(plan, tw, Y, X, [&](int row, int t) { return X[row * TP + t]; }, st_w2);
+    } else if (MODE == 1) {
+        double2 *pb = psi + (size_t)b * L * plane + (size_t)i1 * S2 + t0;
+        fft_run<LT, +1, T, TP, NT>(plan, tw, bufA, bufB, ld_w2, [&](int row, int t, double2 v) {
+            if (t < tmax) pb[row * plane + t] = v;
+        });
+    } else {
+        const double2 *pb = psi + (size_t)b * L * plane + (size_t)i1 * S2 + t0;
+        fft_run<LT, -1, T, TP, NT>(
+            plan, tw, bufA, bufB,
+            [&](int row, int t) { return t < tmax ? pb[row * plane + t] : make_double2(0.0, 0.0); }, st_w2);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ diagonal ops
+// out[b][n] = (f0 + f1 * ke[n]) * C[b][n]
+__global__ void k_diag(const int64_t nG, const int64_t total, const double f0, const double f1,
+                       const double *__restrict__ ke, const double2 *__restrict__ C, double2 *__restrict__ out) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const double f = f0 + f1 * ke[i % nG];
+        const double2 c = C[i];
+        out[i] = make_double2(f * c.x, f * c.y);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ launch helpers
+template <class K>
+cudaError_t ensure_smem(K kernel, size_t bytes) {
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+#define SPEC_SWITCH(L, force_generic, ...)                    \
+    do {                                                      \
+        const int l__ = (force_generic) ? 0 : (L);            \
+        switch (l__) {                                        \
+            case 32: { constexpr int LT = 32; __VA_ARGS__; } break;  \
+            case 64: { constexpr int LT = 64; __VA_ARGS__; } break;  \
+            case 72: { constexpr int LT = 72; __VA_ARGS__; } break;  \
+            case 80: { constexpr int LT = 80; __VA_ARGS__; } break;  \
+            case 128: { constexpr int LT = 128; __VA_ARGS__; } break; \
+            case 216: { constexpr int LT = 216; __VA_ARGS__; } break; \
+            default: { constexpr int LT = 0; __VA_ARGS__; } break;   \
+        }                                                     \
+    } while (0)
+
+struct Bufs {
+    double2 *W1, *W2;
+};
+
+Bufs carve(const jdft_basis *b, int nbatch) {
+    Bufs w;
+    w.W1 = reinterpret_cast<double2 *>(b->ws);
+    w.W2 = w.W1 + (size_t)nbatch * b->ncol * b->S[2];
+    return w;
+}
+
+int launch_cols_inv(const jdft_basis *b, const double2 *C, int nbt, double2 *W1, cudaStream_t st) {
+    const int L = b->S[2];
+    const size_t smem = 2 * (size_t)L * (kT + 1) * sizeof(double2);
+    dim3 grid((b->ncol + kT - 1) / kT, nbt);
+    SPEC_SWITCH(L, b->opt_force_generic, {
+        JDFT_CUDA(ensure_smem(k_cols_inv<LT>, smem));
+        k_cols_inv<LT><<<grid, kNT, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+    });
+    JDFT_LAUNCH_CHECK("k_cols_inv");
+    return JDFT_OK;
+}
+
+int launch_cols_fwd(const jdft_basis *b, const double2 *W1, int nbt, double scale, double kin, const double2 *C,
+                    double2 *out, cudaStream_t st) {
+    const int L = b->S[2];
+    const size_t smem = 2 * (size_t)L * (kT + 1) * sizeof(double2);
+    dim3 grid((b->ncol + kT - 1) / kT, nbt);
+    SPEC_SWITCH(L, b->opt_force_generic, {
+        JDFT_CUDA(ensure_smem(k_cols_fwd<LT>, smem));
+        k_cols_fwd<LT><<<grid, kNT, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
+                                                scale, kin, b->d_ke, C, out);
+    });
+    JDFT_LAUNCH_CHECK("k_cols_fwd");
+    return JDFT_OK;
+}
+
+template <bool FWD>
+int launch_rows(const jdft_basis *b, int nbt, double2 *W1, double2 *W2, cudaStream_t st) {
+    const int L = b->S[1];
+    const size_t smem = 2 * (size_t)L * kT * sizeof(double2) + (size_t)L * sizeof(int);
+    dim3 grid((b->S[2] + kT - 1) / kT, b->npl, nbt);
+    SPEC_SWITCH(L, b->opt_force_generic, {
+        JDFT_CUDA(ensure_smem(k_rows<LT, FWD>, smem));
+        k_rows<LT, FWD><<<grid, kNT, smem, st>>>(b->plan[1], b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
+    });
+    JDFT_LAUNCH_CHECK("k_rows");
+    return JDFT_OK;
+}
+
+template <int MODE>
+int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, double2 *psi, cudaStream_t st) {
+    const int L = b->S[0];
+    const size_t smem = 2 * (size_t)L * kT * sizeof(double2) + (size_t)L * sizeof(int);
+    dim3 grid((b->S[2] + kT - 1) / kT, b->S[1], nbt);
+    SPEC_SWITCH(L, b->opt_force_generic, {
+        JDFT_CUDA(ensure_smem(k_planes<LT, MODE>, smem));
+        k_planes<LT, MODE><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V, psi);
+    });
+    JDFT_LAUNCH_CHECK("k_planes");
+    return JDFT_OK;
+}
+
+int check_common(const jdft_basis *b, const void *in, const void *out, int nb, const char *who) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "%s: null basis", who);
+    if (nb < 0) return jdft_fail(JDFT_EINVAL, "%s: negative band count", who);
+    if (nb > 0 && (!in || !out)) return jdft_fail(JDFT_EINVAL, "%s: null data pointer", who);
+    if ((((uintptr_t)in) | ((uintptr_t)out)) & 15) return jdft_fail(JDFT_EINVAL, "%s: data pointer not 16-byte aligned", who);
+    return JDFT_OK;
+}
+
+}  // namespace
+
+// HC = I^+ (Vloc .* I C) + Omega ke C  for all nb bands, in band batches
+int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C_, int nb, double *HC_, cudaStream_t st) {
+    const int nbatch = jdft_band_batch(b, nb);
+    if (nb > 0 && nbatch == 0) return jdft_fail(JDFT_EWORKSPACE, "apply_H: workspace missing or smaller than one band (%zu bytes)", jdft_fft_bytes_per_band(b));
+    const double2 *C = reinterpret_cast<const double2 *>(C_);
+    double2 *HC = reinterpret_cast<double2 *>(HC_);
+    int rc;
+    for (int b0 = 0; b0 < nb; b0 += nbatch) {
+        const int nbt = nb - b0 < nbatch ? nb - b0 : nbatch;
+        const Bufs w = carve(b, nbatch);
+        const double2 *Cb = C + (size_t)b0 * b->nG;
+        if ((rc = launch_cols_inv(b, Cb, nbt, w.W1, st))) return rc;
+        if ((rc = launch_rows<false>(b, nbt, w.W1, w.W2, st))) return rc;
+        if ((rc = launch_planes<0>(b, nbt, w.W2, Vloc, nullptr, st))) return rc;
+        if ((rc = launch_rows<true>(b, nbt, w.W1, w.W2, st))) return rc;
+        if ((rc = launch_cols_fwd(b, w.W1, nbt, 1.0, b->volume, Cb, HC + (size_t)b0 * b->nG, st))) return rc;
+    }
+    return JDFT_OK;
+}
+
+extern "C" int jdft_apply_I(const jdft_basis *b, const double *C_, int nb, double *psi_, jdft_stream s) {
+    int rc = check_common(b, C_, psi_, nb, "apply_I");
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)s;
+    const int nbatch = jdft_band_batch(b, nb);
+    if (nb > 0 && nbatch == 0) return jdft_fail(JDFT_EWORKSPACE, "apply_I: workspace missing or smaller than one band");
+    const double2 *C = reinterpret_cast<const double2 *>(C_);
+    double2 *psi = reinterpret_cast<double2 *>(psi_);
+    for (int b0 = 0; b0 < nb; b0 += nbatch) {
+        const int nbt = nb - b0 < nbatch ? nb - b0 : nbatch;
+        const Bufs w = carve(b, nbatch);
+        if ((rc = launch_cols_inv(b, C + (size_t)b0 * b->nG, nbt, w.W1, st))) return rc;
+        if ((rc = launch_rows<false>(b, nbt, w.W1, w.W2, st))) return rc;
+        if ((rc = launch_planes<1>(b, nbt, w.W2, nullptr, psi + (size_t)b0 * b->N, st))) return rc;
+    }
+    return JDFT_OK;
+}
+
+static int idag_scaled(const jdft_basis *b, const double *psi_, int nb, double *C_, double scale, jdft_stream s,
+                       const char *who) {
+    int rc = check_common(b, psi_, C_, nb, who);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)s;
+    const int nbatch = jdft_band_batch(b, nb);
+    if (nb > 0 && nbatch == 0) return jdft_fail(JDFT_EWORKSPACE, "%s: workspace missing or smaller than one band", who);
+    double2 *psi = reinterpret_cast<double2 *>(const_cast<double *>(psi_));
+    double2 *C = reinterpret_cast<double2 *>(C_);
+    for (int b0 = 0; b0 < nb; b0 += nbatch) {
+        const int nbt = nb - b0 < nbatch ? nb - b0 : nbatch;
+        const Bufs w = carve(b, nbatch);
+        if ((rc = launch_planes<2>(b, nbt, w.W2, nullptr, psi + (size_t)b0 * b->N, st))) return rc;
+        if ((rc = launch_rows<true>(b, nbt, w.W1, w.W2, st))) return rc;
+        if ((rc = launch_cols_fwd(b, w.W1, nbt, scale, 0.0, C + (size_t)b0 * b->nG, C + (size_t)b0 * b->nG, st))) return rc;
+    }
+    return JDFT_OK;
+}
+
+extern "C" int jdft_apply_Idag(const jdft_basis *b, const double *psi, int nb, double *C, jdft_stream s) {
+    return idag_scaled(b, psi, nb, C, 1.0, s, "apply_Idag");
+}
+
+extern "C" int jdft_apply_J(const jdft_basis *b, const double *psi, int nb, double *C, jdft_stream s) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "apply_J: null basis");
+    return idag_scaled(b, psi, nb, C, 1.0 / (double)b->N, s, "apply_J");
+}
+
+static int diag_op(const jdft_basis *b, const double *C, int nb, double *out, double f0, double f1, jdft_stream s,
+                   const char *who) {
+    int rc = check_common(b, C, out, nb, who);
+    if (rc) return rc;
+    const int64_t total = (int64_t)nb * b->nG;
+    if (total == 0) return JDFT_OK;
+    int64_t blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k_diag<<<(int)blocks, 256, 0, (cudaStream_t)s>>>(b->nG, total, f0, f1, b->d_ke, reinterpret_cast<const double2 *>(C),
+                                                      reinterpret_cast<double2 *>(out));
+    JDFT_LAUNCH_CHECK(who);
+    return JDFT_OK;
+}
+
+extern "C" int jdft_apply_L(const jdft_basis *b, const double *C, int nb, double *LC, jdft_stream s) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "apply_L: null basis");
+    return diag_op(b, C, nb, LC, 0.0, -2.0 * b->volume, s, "apply_L");
+}
+
+extern "C" int jdft_apply_O(const jdft_basis *b, const double *C, int nb, double *OC, jdft_stream s) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "apply_O: null basis");
+    return diag_op(b, C, nb, OC, b->volume, 0.0, s, "apply_O");
+}

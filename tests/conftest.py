@@ -18,3 +18,20 @@ def ref():
     from oracle import ref as _ref
     _ref.lib()
     return _ref
+
+
+def _have_cuda():
+    try:
+        import torch
+        return torch.cuda.is_available()
+    except Exception:
+        return False
+
+
+@pytest.fixture(scope="session")
+def jd():
+    """The CUDA binding (paper_1708_03621_b200.binding).  GPU tests only; fails loudly if the library is missing."""
+    if not _have_cuda():
+        pytest.skip("no CUDA device")
+    import paper_1708_03621_b200.binding as binding
+    return binding

@@ -1,0 +1,246 @@
+"""GPU parity: every exported call of libjdft_b200 (through the C ABI / ctypes binding) against the CPU oracle on
+the same seeded inputs, element by element.  Acceptance (BASELINE.json north_star; reading 18):
+per-band relative L2 error <= 1e-10 in fp64; index maps bit-exact.
+"""
+import numpy as np
+import pytest
+import torch
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def rel_err_per_band(got, want):
+    got = np.asarray(got).reshape(got.shape[0], -1)
+    want = np.asarray(want).reshape(want.shape[0], -1)
+    num = np.linalg.norm(got - want, axis=1)
+    den = np.linalg.norm(want, axis=1)
+    den = np.where(den == 0, 1.0, den)
+    return float(np.max(num / den))
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+class Case:
+    """One (config, k-point): oracle basis + GPU basis + seeded inputs (nb bands)."""
+
+    def __init__(self, ref, jd, cfg_id, ik=0, nb=None, batch=None):
+        R, kpts, Ecut, S = workloads.lattice(cfg_id)
+        self.rb = ref.RefBasis(R, kpts[ik], Ecut, S)
+        self.gb = jd.jdft_basis_create(R, kpts[ik], Ecut, S)
+        inp = workloads.make_inputs(cfg_id, self.rb.iG, ik=ik, nb=nb)
+        self.C, self.V, self.P, self.D = inp["C"], inp["Vloc"], inp["P"], inp["D"]
+        self.nb = self.C.shape[0]
+        jd.jdft_alloc_workspace(self.gb, batch if batch else min(self.nb, 8), max(self.nb, self.P.shape[0]))
+
+
+SMALL = [101, 102, 103, 104, 105, 1]
+
+
+@pytest.fixture(scope="module", params=SMALL)
+def case(request, ref, jd):
+    return Case(ref, jd, request.param)
+
+
+# ------------------------------------------------------------------------------------------ basis (bit-exact)
+
+@pytest.mark.parametrize("cfg_id,ik", [(c, 0) for c in SMALL] + [(103, 1), (2, 0), (3, 0), (4, 0), (4, 1), (4, 2), (4, 3), (5, 0)])
+def test_basis_bit_exact(ref, jd, cfg_id, ik):
+    R, kpts, Ecut, S = workloads.lattice(cfg_id)
+    rb = ref.RefBasis(R, kpts[ik], Ecut, S)
+    gb = jd.jdft_basis_create(R, kpts[ik], Ecut, S)
+    iG, index, ke = jd.jdft_basis_export(gb)
+    assert gb.nG == rb.nG and gb.N == rb.N
+    assert np.array_equal(iG, rb.iG)
+    assert np.array_equal(index, rb.index)
+    assert np.max(np.abs(ke - rb.ke)) <= 1e-14 * np.max(rb.ke)
+    assert abs(gb.volume - rb.volume) <= 1e-14 * rb.volume
+
+
+def test_basis_errors(jd):
+    R = np.diag([10.0, 10.0, 10.0])
+    with pytest.raises(jd.JdftError) as e:
+        jd.jdft_basis_create(R, [0, 0, 0], 10.0, (14, 32, 32))     # 14 = 2 * 7
+    assert e.value.code == jd.JDFT_EBOX
+    with pytest.raises(jd.JdftError) as e:
+        jd.jdft_basis_create(R, [0, 0, 0], 10.0, (8, 32, 32))      # sphere spans -7..7 > 8
+    assert e.value.code == jd.JDFT_EBOX
+    with pytest.raises(jd.JdftError) as e:
+        jd.jdft_basis_create(np.zeros((3, 3)), [0, 0, 0], 10.0, (32, 32, 32))
+    assert e.value.code == jd.JDFT_EINVAL
+    with pytest.raises(jd.JdftError) as e:
+        jd.jdft_basis_create(R, [0, 0, 0], -1.0, (32, 32, 32))
+    assert e.value.code == jd.JDFT_EINVAL
+
+
+def test_workspace_errors(ref, jd):
+    R, kpts, Ecut, S = workloads.lattice(101)
+    gb = jd.jdft_basis_create(R, kpts[0], Ecut, S)
+    C = torch.zeros((2, gb.nG), dtype=torch.complex128, device="cuda")
+    with pytest.raises(jd.JdftError) as e:
+        jd.jdft_apply_I(gb, C)
+    assert e.value.code == jd.JDFT_EWORKSPACE
+    jd.jdft_set_workspace(gb, torch.empty(64, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(jd.JdftError) as e:
+        jd.jdft_apply_I(gb, C)
+    assert e.value.code == jd.JDFT_EWORKSPACE
+    with pytest.raises(jd.JdftError) as e:
+        jd.jdft_set_option(gb, "no_such_option", 1)
+    assert e.value.code == jd.JDFT_EINVAL
+
+
+# ------------------------------------------------------------------------------------------ operators
+
+def test_apply_I(case, jd):
+    want = case.rb.apply_I(case.C)
+    got = jd.jdft_apply_I(case.gb, dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+
+
+def test_apply_Idag_and_J(case, jd):
+    rng = np.random.default_rng(5)
+    nb = min(case.nb, 6)
+    psi = rng.standard_normal((nb,) + case.rb.shape) + 1j * rng.standard_normal((nb,) + case.rb.shape)
+    want = case.rb.apply_Idag(psi)
+    got = jd.jdft_apply_Idag(case.gb, dev(psi)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+    wantJ = case.rb.apply_J(psi)
+    gotJ = jd.jdft_apply_J(case.gb, dev(psi)).cpu().numpy()
+    assert rel_err_per_band(gotJ, wantJ) <= TOL
+
+
+def test_apply_L_O(case, jd):
+    C = dev(case.C)
+    assert rel_err_per_band(jd.jdft_apply_L(case.gb, C).cpu().numpy(), case.rb.apply_L(case.C)) <= 1e-14
+    assert rel_err_per_band(jd.jdft_apply_O(case.gb, C).cpu().numpy(), case.rb.apply_O(case.C)) <= 1e-14
+    # in place
+    C2 = C.clone()
+    jd.jdft_apply_L(case.gb, C2, C2)
+    assert rel_err_per_band(C2.cpu().numpy(), case.rb.apply_L(case.C)) <= 1e-14
+
+
+def test_project(case, jd):
+    want = case.rb.project(case.P, case.C)
+    got = jd.jdft_project(case.gb, dev(case.P), dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+
+
+def test_apply_Vnl_diag(case, jd):
+    want = case.rb.apply_Vnl(case.P, case.D, case.C)
+    got = jd.jdft_apply_Vnl(case.gb, dev(case.P), dev(case.D), dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+    # accumulate into an existing array
+    base = np.ascontiguousarray(case.C[::-1]) * 0.37
+    out = dev(base)
+    jd.jdft_apply_Vnl(case.gb, dev(case.P), dev(case.D), dev(case.C), out, accumulate=True)
+    assert rel_err_per_band(out.cpu().numpy(), base + want) <= TOL
+
+
+def test_apply_Vnl_dense_D(case, jd):
+    rng = np.random.default_rng(11)
+    n = case.P.shape[0]
+    A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    D = (A + A.conj().T) / 2
+    want = case.rb.apply_Vnl(case.P, D, case.C)
+    got = jd.jdft_apply_Vnl(case.gb, dev(case.P), dev(D), dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+
+
+def test_apply_H_full(case, jd):
+    want = case.rb.apply_H(case.V, case.P, case.D, case.C)
+    got = jd.jdft_apply_H(case.gb, dev(case.V.reshape(-1)), dev(case.P), dev(case.D), dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+
+
+def test_apply_H_local_only(case, jd):
+    want = case.rb.apply_H(case.V, None, None, case.C)
+    got = jd.jdft_apply_H(case.gb, dev(case.V.reshape(-1)), None, None, dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+
+
+def test_apply_H_zero_V(case, jd):
+    V0 = np.zeros_like(case.V)
+    want = case.rb.apply_H(V0, case.P, case.D, case.C)
+    got = jd.jdft_apply_H(case.gb, dev(V0.reshape(-1)), dev(case.P), dev(case.D), dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+
+
+def test_overlap(case, jd):
+    rng = np.random.default_rng(3)
+    C2 = case.C[: max(1, case.nb // 2)] + 0.1 * (rng.standard_normal((max(1, case.nb // 2), case.rb.nG)) + 0j)
+    want = case.rb.overlap(case.C, C2)                      # [nb1, nb2]
+    got = jd.jdft_overlap(case.gb, dev(case.C), dev(C2)).cpu().numpy()
+    assert got.shape == want.shape
+    assert rel_err_per_band(got.T, want.T) <= TOL           # per column of M
+
+
+def test_host_variants(case, jd):
+    want = case.rb.apply_H(case.V, case.P, case.D, case.C)
+    HC = torch.empty(case.C.shape, dtype=torch.complex128).pin_memory()
+    jd.jdft_apply_H_host(case.gb, torch.from_numpy(case.V.reshape(-1).copy()), torch.from_numpy(case.P),
+                         torch.from_numpy(case.D), torch.from_numpy(case.C), HC)
+    assert rel_err_per_band(HC.numpy(), want) <= TOL
+    M = torch.empty((case.nb, case.nb), dtype=torch.complex128)
+    got = jd.jdft_overlap_host(case.gb, torch.from_numpy(case.C), torch.from_numpy(case.C), M).numpy()
+    assert rel_err_per_band(got.T, case.rb.overlap(case.C, case.C).T) <= TOL
+
+
+# ------------------------------------------------------------------------------------------ GPU-side properties
+
+def test_generic_fft_path_matches(ref, jd):
+    """Lengths with specialised kernels (32, 64) also run on the runtime-radix kernels; both must match the oracle."""
+    for cfg_id in (1, 104):
+        c = Case(ref, jd, cfg_id, nb=4)
+        want = c.rb.apply_H(c.V, c.P, c.D, c.C)
+        args = (dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C))
+        a = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+        jd.jdft_set_option(c.gb, "force_generic_fft", 1)
+        b = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+        assert rel_err_per_band(a, want) <= TOL and rel_err_per_band(b, want) <= TOL
+        assert rel_err_per_band(a, b) <= 1e-13
+
+
+def test_band_batch_independence(ref, jd):
+    c = Case(ref, jd, 102)
+    args = (dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C))
+    outs = []
+    for batch in (1, 3, 7, 19):
+        jd.jdft_set_option(c.gb, "band_batch", batch)
+        outs.append(jd.jdft_apply_H(c.gb, *args).cpu().numpy())
+    for o in outs[1:]:
+        assert rel_err_per_band(o, outs[0]) <= 1e-13
+
+
+def test_gpu_J_I_identity_and_hermiticity(case, jd):
+    C = dev(case.C)
+    back = jd.jdft_apply_J(case.gb, jd.jdft_apply_I(case.gb, C)).cpu().numpy()
+    assert rel_err_per_band(back, case.C) <= 1e-13
+    rng = np.random.default_rng(9)
+    a = rng.standard_normal((1, case.rb.nG)) + 1j * rng.standard_normal((1, case.rb.nG))
+    b = rng.standard_normal((1, case.rb.nG)) + 1j * rng.standard_normal((1, case.rb.nG))
+    args = (dev(case.V.reshape(-1)), dev(case.P), dev(case.D))
+    Ha = jd.jdft_apply_H(case.gb, *args, dev(a)).cpu().numpy()
+    Hb = jd.jdft_apply_H(case.gb, *args, dev(b)).cpu().numpy()
+    lhs = np.vdot(a, Hb)
+    rhs = np.conj(np.vdot(b, Ha))
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(a) * np.linalg.norm(Hb)
+
+
+def test_empty_inputs(case, jd):
+    C0 = torch.empty((0, case.gb.nG), dtype=torch.complex128, device="cuda")
+    assert jd.jdft_apply_H(case.gb, dev(case.V.reshape(-1)), dev(case.P), dev(case.D), C0).shape[0] == 0
+    assert jd.jdft_apply_L(case.gb, C0).shape[0] == 0
+    # no projectors: Vnl writes zeros
+    out = jd.jdft_apply_Vnl(case.gb, None, None, dev(case.C))
+    assert float(out.abs().max()) == 0.0
+
+
+def test_launch_counter(case, jd):
+    jd.jdft_launch_count(reset=True)
+    jd.jdft_apply_H(case.gb, dev(case.V.reshape(-1)), dev(case.P), dev(case.D), dev(case.C))
+    assert jd.jdft_launch_count() >= 8

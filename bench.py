@@ -1,0 +1,407 @@
+#!/usr/bin/env python
+"""bench.py -- H.psi band-applications/s (fp64) of libjdft_b200 on one BASELINE.json workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over the workload: jdft_apply_H on every band of every k-point of the
+config (config 5 also runs its 512 x 512 jdft_overlap).  Inputs are seeded synthetic data of BASELINE.json's
+shapes (workloads/), resident in HBM before the timed region.  L2 is flushed (a 512 MiB memset) before every
+timed step; steps are timed with CUDA events on the launch stream; N > 1 runs N independent replicas
+("replicas only") and takes the max over ranks.  Prints ONE JSON line (rank 0).
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded band sample of the
+same workload and prints the same line with "impl": "reference".
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "H.psi band-applications/s (fp64)"
+UNIT = "band-applications/s"
+KERNELS = ["cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd", "gemm_dotk", "gemm_expand", "splitk_reduce"]
+HBM_KERNELS = {"cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd", "splitk_reduce"}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def fp64_peak():
+    """Live DMMA / DFMA peak of this GPU from the committed micro-benchmark (csrc/fp64_peak.cu)."""
+    tool = os.path.join(ROOT, "paper_1708_03621_b200", "fp64_peak")
+    try:
+        out = subprocess.run([tool], capture_output=True, text=True, timeout=120).stdout.strip().splitlines()[-1]
+        d = json.loads(out)
+        return float(d["dmma_tflops"]), float(d["dfma_tflops"]), "measured (csrc/fp64_peak.cu DMMA micro-benchmark, this run)"
+    except Exception:
+        return 37.2, 37.2, "nominal (148 SM x 64 FMA/clk x 2 x 1.965 GHz; micro-benchmark unavailable)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.FIELDS,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, parts[2:6]):
+                if v == "Active":
+                    reasons.add(nme)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out["sm_mhz"] = float(np.median(sm))
+            out["sm_max_mhz"] = float(max(mx))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def config_sizes(cfg_id):
+    cfg = workloads.get_config(cfg_id)
+    return cfg, len(cfg["kpoints"]), cfg["nb"], cfg["natoms"] * cfg["n_lm"]
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+
+def run_reference(args):
+    from oracle import ref
+    cfg, nk, nb, nproj = config_sizes(args.config)
+    R, kpts, Ecut, S = workloads.lattice(args.config)
+    threads = ref.threads()
+    rb = ref.RefBasis(R, kpts[0], Ecut, S)
+    inp = workloads.make_inputs(args.config, rb.iG, ik=0, nb=max(threads, 1) * 4)
+    C = inp["C"]
+    # calibrate: one band per thread, then size the per-step sample so the whole run stays within a few minutes
+    t0 = time.perf_counter()
+    rb.apply_H(inp["Vloc"], inp["P"], inp["D"], C[:threads])
+    t1 = time.perf_counter() - t0
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    nsample = int(max(threads, min(C.shape[0], threads * max(1, int(budget / max(t1, 1e-3))))))
+    nsample = (nsample // threads) * threads
+    Cs = np.ascontiguousarray(C[:nsample])
+    for _ in range(args.warmup):
+        rb.apply_H(inp["Vloc"], inp["P"], inp["D"], Cs)
+    times = []
+    for _ in range(args.steps):
+        t0 = time.perf_counter()
+        rb.apply_H(inp["Vloc"], inp["P"], inp["D"], Cs)
+        times.append(time.perf_counter() - t0)
+    ms = 1e3 * float(np.mean(times))
+    value = nsample / (ms * 1e-3)
+    sample = "%d bands of k-point 0 of config %d per step (full P, Vloc; apply_H only)" % (nsample, args.config)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "bands_per_step": nsample, "nproj": nproj, "fft_box": list(S)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(cfg_id, seconds=15.0):
+    """The oracle, as it stands, on a bounded sample (~10-30 s of CPU work) of the same workload."""
+    from oracle import ref
+    R, kpts, Ecut, S = workloads.lattice(cfg_id)
+    threads = ref.threads()
+    rb = ref.RefBasis(R, kpts[0], Ecut, S)
+    inp = workloads.make_inputs(cfg_id, rb.iG, ik=0, nb=threads * 8)
+    t0 = time.perf_counter()
+    rb.apply_H(inp["Vloc"], inp["P"], inp["D"], inp["C"][:threads])
+    t1 = time.perf_counter() - t0
+    rounds = int(max(1, min(8, seconds / max(t1, 1e-3))))
+    n = threads * rounds
+    t0 = time.perf_counter()
+    rb.apply_H(inp["Vloc"], inp["P"], inp["D"], inp["C"][:n])
+    dt = time.perf_counter() - t0
+    return {"value": n / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "%d bands of k-point 0 of config %d, jdft_ref_apply_H, %.1f s wall on %d threads" % (n, cfg_id, dt, threads)}
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+
+def algorithmic(cfgk, kernel, nbatches):
+    """Algorithmic bytes (HBM kernels) or flops (GEMMs) of ONE step for one k-point."""
+    nG, a, b, N, nb, npj = cfgk["nG"], cfgk["a"], cfgk["b"], cfgk["N"], cfgk["nb"], cfgk["nproj"]
+    if kernel == "cols_inv":
+        return nb * 16 * (nG + a)
+    if kernel in ("rows_inv", "rows_fwd"):
+        return nb * 16 * (a + b)
+    if kernel == "planes":
+        return nb * 32 * b + nbatches * 8 * N
+    if kernel == "cols_fwd":
+        return nb * (16 * (a + 2 * nG) + 8 * nG)
+    if kernel == "gemm_dotk":
+        return 8 * nb * npj * nG + cfgk["overlap_flops"]
+    if kernel == "gemm_expand":
+        return 8 * nb * npj * nG
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1708_03621_b200.binding as jd
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    cfg, nk, nb, nproj = config_sizes(args.config)
+    R, kpts, Ecut, S = workloads.lattice(args.config)
+    do_overlap = args.config == 5
+    atoms = workloads.atoms_fractional(args.config)
+    Vh = workloads.make_vloc(args.config, atoms).reshape(-1)
+    V = torch.from_numpy(Vh).cuda()
+    D_h = workloads.make_D(args.config)
+    D = torch.from_numpy(D_h).cuda()
+    ks = []
+    for ik in range(nk):
+        gb = jd.jdft_basis_create(R, kpts[ik], Ecut, S, device=local)
+        iG, _, _ = jd.jdft_basis_export(gb)
+        C_h = workloads.make_bands(args.config, gb.nG, ik=ik)
+        P_h = workloads.make_projectors(args.config, iG, kpts[ik], atoms)
+        jd.jdft_alloc_workspace(gb, max(args.batch, 16), max(nb, nproj))
+        if args.batch > 0:
+            jd.jdft_set_option(gb, "band_batch", args.batch)
+        ks.append(dict(gb=gb, C=torch.from_numpy(C_h).cuda(), P=torch.from_numpy(P_h).cuda(),
+                       HC=torch.empty((nb, gb.nG), dtype=torch.complex128, device="cuda"),
+                       M=torch.empty((nb, nb), dtype=torch.complex128, device="cuda") if do_overlap else None,
+                       C_h=C_h, P_h=P_h,
+                       info=dict(nG=gb.nG, a=gb.ncol * S[2], b=gb.npl * S[1] * S[2], N=gb.N, nb=nb, nproj=nproj,
+                                 overlap_flops=8 * nb * nb * gb.nG if do_overlap else 0)))
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+
+    def step():
+        for k in ks:
+            jd.jdft_apply_H(k["gb"], V, k["P"], D, k["C"], k["HC"])
+            if do_overlap:
+                jd.jdft_overlap(k["gb"], k["C"], k["C"], k["M"])
+
+    def timed(nsteps):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nsteps)]
+        for a, b in ev:
+            flush.zero_()
+            a.record()
+            step()
+            b.record()
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    # warm-up; the per-kernel profile (events around every launch of one kernel at a time) runs inside it
+    timed(max(args.warmup, 3))
+    per_kernel = {}
+    nbatches = {}
+    for name in KERNELS:
+        tot, launches = 0.0, 0
+        for k in ks:
+            jd.jdft_set_option(k["gb"], "profile_kernel", jd.KERNEL_IDS[name])
+        flush.zero_()
+        step()
+        for k in ks:
+            n, ms = jd.jdft_profile_read(k["gb"])
+            tot += ms
+            launches += n
+            jd.jdft_set_option(k["gb"], "profile_kernel", 0)
+        per_kernel[name] = (tot, launches)
+        nbatches[name] = launches
+    dominant = max(per_kernel, key=lambda n: per_kernel[n][0])
+
+    # timed region: K steps, events around each; the dominant kernel's launches are bracketed by events inside it
+    for k in ks:
+        jd.jdft_set_option(k["gb"], "profile_kernel", jd.KERNEL_IDS[dominant])
+        jd.jdft_profile_read(k["gb"])
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    jd.jdft_launch_count(reset=True)
+    sampler = ClockSampler(local) if rank == 0 else None
+    t_wall = time.perf_counter()
+    times = timed(args.steps)
+    t_wall = time.perf_counter() - t_wall
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    launches = jd.jdft_launch_count()
+    dom_ms, dom_n = 0.0, 0
+    for k in ks:
+        n, ms = jd.jdft_profile_read(k["gb"])
+        dom_ms += ms
+        dom_n += n
+        jd.jdft_set_option(k["gb"], "profile_kernel", 0)
+    ms_step = float(np.mean(times))
+    if world > 1:
+        t = torch.tensor([ms_step], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step = float(t.item())
+    units = nb * nk
+    value = world * units / (ms_step * 1e-3)
+
+    # end to end through the HOST-buffer ABI call: pinned host inputs -> H2D -> kernels -> D2H, every step
+    Vp = torch.from_numpy(Vh).pin_memory()
+    Dp = torch.from_numpy(D_h).pin_memory()
+    host = [dict(C=torch.from_numpy(k["C_h"]).pin_memory(), P=torch.from_numpy(k["P_h"]).pin_memory(),
+                 HC=torch.empty((nb, k["gb"].nG), dtype=torch.complex128).pin_memory(),
+                 M=torch.empty((nb, nb), dtype=torch.complex128).pin_memory() if do_overlap else None) for k in ks]
+
+    def step_host():
+        for k, h in zip(ks, host):
+            jd.jdft_apply_H_host(k["gb"], Vp, h["P"], Dp, h["C"], h["HC"])
+            if do_overlap:
+                jd.jdft_overlap_host(k["gb"], h["C"], h["C"], h["M"])
+
+    step_host()
+    e2e_steps = max(1, min(args.steps, 5))
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        step_host()
+    torch.cuda.synchronize()
+    e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    h2d = sum(h["C"].numel() * 16 + h["P"].numel() * 16 + Vp.numel() * 8 + Dp.numel() * 8 +
+              (2 * h["C"].numel() * 16 if do_overlap else 0) for h in host)
+    d2h = sum(h["HC"].numel() * 16 + (h["M"].numel() * 16 if do_overlap else 0) for h in host)
+
+    if rank != 0:
+        return
+    hbm_peak, hbm_src = measured_peaks()
+    dmma_peak, dfma_peak, fp_src = fp64_peak()
+
+    def roof(name, ms, launches_):
+        if ms <= 0:
+            return None
+        alg = sum(algorithmic(k["info"], name, max(1, launches_ // max(1, len(ks)))) for k in ks)
+        if name in HBM_KERNELS:
+            ach = alg / (ms * 1e-3) / 1e9
+            return {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
+        ach = alg / (ms * 1e-3) / 1e12
+        return {"bound": "tensor", "achieved": ach, "peak": dmma_peak, "unit": "TFLOP/s", "frac": ach / dmma_peak}
+
+    kernels = {}
+    for name, (ms, n) in per_kernel.items():
+        r = roof(name, ms, n)
+        kernels[name] = {"ms_per_step": ms, "launches": n}
+        if r and name != "splitk_reduce":
+            kernels[name].update({"achieved": r["achieved"], "unit": r["unit"], "frac": r["frac"]})
+    roofline = roof(dominant, dom_ms / args.steps, dom_n // args.steps)
+    roofline.update({"kernel": dominant, "launches_per_step": dom_n // args.steps,
+                     "avg_launch_ms": dom_ms / max(1, dom_n), "peak_source": hbm_src if roofline["bound"] == "hbm" else fp_src,
+                     "traffic": None, "share_of_step": dom_ms / args.steps / ms_step})
+    traffic_file = os.path.join(ROOT, "profiles", "traffic_r01.json")
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as f:
+            tr = json.load(f)
+        roofline["traffic"] = tr.get("cfg%d" % args.config, {}).get(dominant)
+    local_bytes = sum(sum(algorithmic(k["info"], n, max(1, nbatches[n] // len(ks))) for n in
+                          ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd")) for k in ks)
+    local_ms = sum(per_kernel[n][0] for n in ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd"))
+    gemm_flops = sum(algorithmic(k["info"], "gemm_dotk", 1) + algorithmic(k["info"], "gemm_expand", 1) for k in ks)
+    gemm_ms = per_kernel["gemm_dotk"][0] + per_kernel["gemm_expand"][0]
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": cfg["name"], "bands": nb, "kpoints": nk, "nproj": nproj, "fft_box": list(S),
+                   "nG": [k["gb"].nG for k in ks], "overlap_in_step": do_overlap, "l2": "flushed (512 MiB memset) before every timed step",
+                   "parallelism": "replicas x%d" % world},
+        "clocks": clocks,
+        "e2e": {"value": world * units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_ms, "steps": e2e_steps},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "groups": {"fft_local": {"GB/s": local_bytes / (local_ms * 1e-3) / 1e9 if local_ms else None,
+                                 "frac_hbm": local_bytes / (local_ms * 1e-3) / 1e9 / hbm_peak if local_ms else None,
+                                 "ms_per_step": local_ms},
+                   "gemm": {"TFLOP/s": gemm_flops / (gemm_ms * 1e-3) / 1e12 if gemm_ms else None,
+                            "frac_fp64_tensor": gemm_flops / (gemm_ms * 1e-3) / 1e12 / dmma_peak if gemm_ms else None,
+                            "ms_per_step": gemm_ms}},
+        "kernels": kernels,
+        "fp64_peaks": {"dmma_tflops": dmma_peak, "dfma_tflops": dfma_peak, "source": fp_src},
+        "wall_s_timed_region": t_wall,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args.config)
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json workload 1..5 (default 2 = configs[1])")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--batch", type=int, default=0, help="bands per FFT batch (0 = automatic)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_reference(args)
+        return
+    run_ours(args)
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

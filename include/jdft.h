@@ -82,7 +82,7 @@ int jdft_basis_device_maps(const jdft_basis *b, const int32_t **index_dev, const
 size_t jdft_workspace_bytes(const jdft_basis *b, int nbands_batch, int nrows_max);
 int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
 /* tunables: "band_batch" (bands per FFT batch, 0 = automatic), "force_generic_fft" (0/1: use the
- * runtime-radix FFT kernels even for lengths that have specialised ones; for tests)                   */
+ * runtime-radix FFT kernels even for lengths that have specialised ones; for tests), "profile_kernel"  */
 int jdft_set_option(jdft_basis *b, const char *key, int64_t value);
 
 /* ---- operators ------------------------------------------------------ */
@@ -120,8 +120,11 @@ int jdft_overlap_host(jdft_basis *b, const double *C1_host, int nb1, const doubl
 const char *jdft_last_error(void);
 /* kernels launched by this thread since the last call with reset != 0 (bench.py's gpu_launches)       */
 int64_t jdft_launch_count(int reset);
-/* per-kernel-group device time of the LAST apply_H / overlap call when "profile" option is on:
- * not part of the hot path.                                                                           */
+/* Diagnostics, off by default: jdft_set_option(b, "profile_kernel", id) brackets every later launch of ONE
+ * kernel (1 cols_inv, 2 rows_inv, 3 planes, 4 rows_fwd, 5 cols_fwd, 6 gemm_dotk, 7 gemm_expand, 8 split-K
+ * reduce, 9 diag; 0 = off) with CUDA events on the launch stream; jdft_profile_read waits for them, returns
+ * the number of launches and their summed device time, and resets.  Not thread-safe.                   */
+int jdft_profile_read(jdft_basis *b, int64_t *launches, double *total_ms);
 const char *jdft_version(void);
 
 #ifdef __cplusplus

@@ -20,7 +20,7 @@ EXPORTS = [
     "jdft_basis_device_maps", "jdft_workspace_bytes", "jdft_set_workspace", "jdft_set_option",
     "jdft_apply_I", "jdft_apply_Idag", "jdft_apply_J", "jdft_apply_L", "jdft_apply_O", "jdft_apply_Vnl",
     "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_H_host", "jdft_overlap_host",
-    "jdft_last_error", "jdft_launch_count", "jdft_version",
+    "jdft_last_error", "jdft_launch_count", "jdft_profile_read", "jdft_version",
 ]
 
 
@@ -57,6 +57,7 @@ def _load():
     L.jdft_last_error.restype = ctypes.c_char_p
     L.jdft_launch_count.argtypes = [ci]
     L.jdft_launch_count.restype = i64
+    L.jdft_profile_read.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(dp)]
     L.jdft_version.restype = ctypes.c_char_p
     return L
 
@@ -293,6 +294,17 @@ def jdft_overlap_host(basis, C1, C2, M):
 
 def jdft_launch_count(reset=False):
     return int(_lib.jdft_launch_count(1 if reset else 0))
+
+
+KERNEL_IDS = {"cols_inv": 1, "rows_inv": 2, "planes": 3, "rows_fwd": 4, "cols_fwd": 5, "gemm_dotk": 6,
+              "gemm_expand": 7, "splitk_reduce": 8, "diag": 9}
+
+
+def jdft_profile_read(basis):
+    """(launches, total_ms) of the kernel selected with jdft_set_option(basis, "profile_kernel", id); resets."""
+    n, ms = ctypes.c_int64(), ctypes.c_double()
+    _chk(_lib.jdft_profile_read(basis._h, ctypes.byref(n), ctypes.byref(ms)))
+    return n.value, ms.value
 
 
 def jdft_version():

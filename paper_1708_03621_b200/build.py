@@ -10,6 +10,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libjdft_b200.so")
+PEAK_TOOL = os.path.join(HERE, "fp64_peak")  # micro-benchmark binary bench.py runs for the FP64 roofline peak
 SOURCES = ["basis.cu", "local.cu", "gemm.cu", "api.cu"]
 HEADERS = [os.path.join(CSRC, "jdft_internal.h"), os.path.join(CSRC, "fft.cuh"),
            os.path.join(HERE, "..", "include", "jdft.h")]
@@ -54,6 +55,11 @@ def build(force=False, verbose=False):
         tmp = LIB + ".tmp%d" % os.getpid()
         run([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", tmp] + objs)  # static cudart (nvcc default)
         os.replace(tmp, LIB)
+    peak_src = os.path.join(CSRC, "fp64_peak.cu")
+    if force or _stale(PEAK_TOOL, [peak_src]):
+        tmp = PEAK_TOOL + ".tmp%d" % os.getpid()
+        run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-Wno-deprecated-gpu-targets", "-o", tmp, peak_src])
+        os.replace(tmp, PEAK_TOOL)
     return LIB
 
 

@@ -35,7 +35,7 @@ int vnl_impl(const jdft_basis *b, const double *P, int nproj, const double *D, i
         Bd = B2;
     }
     // out[ib][n] (+)= sum_j Bd[ib][j] P[j][n]
-    return jdft_gemm_expand(Bd, nb, P, nproj, b->nG, out, accumulate, st);
+    return jdft_gemm_expand(b, Bd, nb, P, nproj, b->nG, out, accumulate, st);
 }
 
 int check_vnl_args(const jdft_basis *b, const double *P, int nproj, const double *D, int D_mode, const double *C, int nb,

@@ -89,6 +89,7 @@ extern "C" int jdft_basis_destroy(jdft_basis *b) {
     cudaFree(b->d_planeof);
     for (int d = 0; d < 3; d++) cudaFree(b->d_tw[d]);
     for (int i = 0; i < 8; i++) cudaFree(b->hb[i]);
+    for (cudaEvent_t e : b->prof_ev) cudaEventDestroy(e);
     delete b;
     return JDFT_OK;
 }
@@ -118,6 +119,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     for (int d = 0; d < 3; d++) b->d_tw[d] = nullptr;
     for (int i = 0; i < 8; i++) { b->hb[i] = nullptr; b->hb_bytes[i] = 0; }
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
+    b->opt_profile_kernel = 0; b->prof_used = 0;
 
     // G = 2 pi R^-1 (adjugate / det): row i of G is the reciprocal vector b_i
     {
@@ -324,6 +326,7 @@ extern "C" int jdft_set_option(jdft_basis *b, const char *key, int64_t value) {
     if (!b || !key) return jdft_fail(JDFT_EINVAL, "set_option: null argument");
     if (!strcmp(key, "band_batch")) { b->opt_band_batch = value < 0 ? 0 : value; return JDFT_OK; }
     if (!strcmp(key, "force_generic_fft")) { b->opt_force_generic = value != 0; return JDFT_OK; }
+    if (!strcmp(key, "profile_kernel")) { b->opt_profile_kernel = value; b->prof_used = 0; return JDFT_OK; }
     return jdft_fail(JDFT_EINVAL, "set_option: unknown key '%s'", key);
 }
 
@@ -343,4 +346,43 @@ int jdft_band_batch(const jdft_basis *b, int nb) {
     if (want > nb) want = nb;
     if (want < 1) want = 1;
     return (int)want;
+}
+
+// ---- optional per-kernel event timing (diagnostics; not thread-safe; off by default) ------------------
+
+void jdft_prof_begin(const jdft_basis *cb, int kid, cudaStream_t st) {
+    if (cb->opt_profile_kernel != kid) return;
+    jdft_basis *b = const_cast<jdft_basis *>(cb);
+    if (b->prof_used + 2 > b->prof_ev.size()) {
+        if (b->prof_ev.size() >= 1 << 16) return;
+        for (int i = 0; i < 2; i++) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return;
+            b->prof_ev.push_back(e);
+        }
+    }
+    cudaEventRecord(b->prof_ev[b->prof_used], st);
+}
+
+void jdft_prof_end(const jdft_basis *cb, int kid, cudaStream_t st) {
+    if (cb->opt_profile_kernel != kid) return;
+    jdft_basis *b = const_cast<jdft_basis *>(cb);
+    if (b->prof_used + 2 > b->prof_ev.size()) return;
+    cudaEventRecord(b->prof_ev[b->prof_used + 1], st);
+    b->prof_used += 2;
+}
+
+extern "C" int jdft_profile_read(jdft_basis *b, int64_t *launches, double *total_ms) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "profile_read: null basis");
+    double ms = 0.0;
+    for (size_t i = 0; i + 1 < b->prof_used; i += 2) {
+        JDFT_CUDA(cudaEventSynchronize(b->prof_ev[i + 1]));
+        float t = 0.f;
+        JDFT_CUDA(cudaEventElapsedTime(&t, b->prof_ev[i], b->prof_ev[i + 1]));
+        ms += t;
+    }
+    if (launches) *launches = (int64_t)(b->prof_used / 2);
+    if (total_ms) *total_ms = ms;
+    b->prof_used = 0;
+    return JDFT_OK;
 }

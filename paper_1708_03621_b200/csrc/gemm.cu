@@ -246,7 +246,6 @@ cudaError_t ensure_smem(K kernel, size_t bytes) {
 int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y, int Cn, int64_t K, int conjY,
                    double scale, const double *dscale, double *Out, void *scratch, size_t scratch_bytes,
                    cudaStream_t st) {
-    (void)b;
     if (Rn <= 0 || Cn <= 0) return JDFT_OK;
     const int64_t ktiles = (K + BK - 1) / BK;
     const int tiles = ((Rn + BM - 1) / BM) * ((Cn + BN - 1) / BN);
@@ -262,6 +261,7 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     if (nsplit < 1) nsplit = 1;
     const size_t smem = 2 * STAGES * OPK_BYTES;
     dim3 grid((Cn + BN - 1) / BN, (Rn + BM - 1) / BM, (unsigned)nsplit);
+    jdft_prof_begin(b, JDFT_K_GEMM_DOTK, st);
     if (conjY) {
         JDFT_CUDA(ensure_smem(k_gemm_dotk<true>, smem));
         k_gemm_dotk<true><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
@@ -269,22 +269,27 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
         JDFT_CUDA(ensure_smem(k_gemm_dotk<false>, smem));
         k_gemm_dotk<false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
     }
+    jdft_prof_end(b, JDFT_K_GEMM_DOTK, st);
     JDFT_LAUNCH_CHECK("k_gemm_dotk");
     const int64_t total = (int64_t)Rn * Cn;
     int64_t blocks = (total + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
+    jdft_prof_begin(b, JDFT_K_REDUCE, st);
     k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, total, Cn, scale, dscale, (double2 *)Out);
+    jdft_prof_end(b, JDFT_K_REDUCE, st);
     JDFT_LAUNCH_CHECK("k_splitk_reduce");
     return JDFT_OK;
 }
 
-int jdft_gemm_expand(const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
+int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
                      cudaStream_t st) {
     if (Rn <= 0 || Nn <= 0) return JDFT_OK;
     const size_t smem = STAGES * (OPK_BYTES + OPN_BYTES);
     JDFT_CUDA(ensure_smem(k_gemm_expand, smem));
     dim3 grid((unsigned)((Nn + BN - 1) / BN), (Rn + BM - 1) / BM);
+    jdft_prof_begin(b, JDFT_K_GEMM_EXPAND, st);
     k_gemm_expand<<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, accumulate);
+    jdft_prof_end(b, JDFT_K_GEMM_EXPAND, st);
     JDFT_LAUNCH_CHECK("k_gemm_expand");
     return JDFT_OK;
 }

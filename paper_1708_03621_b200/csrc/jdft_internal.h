@@ -41,10 +41,20 @@ struct jdft_basis {
     size_t ws_bytes;
     // options
     int64_t opt_band_batch, opt_force_generic;
+    // optional per-kernel event timing (option "profile_kernel" = one of JDFT_K_*; 0 = off).  Diagnostics only.
+    int64_t opt_profile_kernel;
+    std::vector<cudaEvent_t> prof_ev;  // pairs (begin, end)
+    size_t prof_used;
     // cached device buffers of the *_host entry points (library-owned, grow-only)
     void *hb[8];
     size_t hb_bytes[8];
 };
+
+// kernel ids for the "profile_kernel" option
+enum { JDFT_K_NONE = 0, JDFT_K_COLS_INV = 1, JDFT_K_ROWS_INV = 2, JDFT_K_PLANES = 3, JDFT_K_ROWS_FWD = 4,
+       JDFT_K_COLS_FWD = 5, JDFT_K_GEMM_DOTK = 6, JDFT_K_GEMM_EXPAND = 7, JDFT_K_REDUCE = 8, JDFT_K_DIAG = 9 };
+void jdft_prof_begin(const jdft_basis *b, int kid, cudaStream_t st);
+void jdft_prof_end(const jdft_basis *b, int kid, cudaStream_t st);
 
 // error plumbing
 int jdft_fail(int code, const char *fmt, ...);
@@ -76,5 +86,5 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
                    double scale, const double *dscale, double *Out, void *scratch, size_t scratch_bytes,
                    cudaStream_t st);
 // Out[r][n] (+)= sum_j A[r][j] * Pm[j][n];  A [Rn][K] (K contiguous), Pm [K][Nn] (n contiguous), Out [Rn][Nn]
-int jdft_gemm_expand(const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
+int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
                      cudaStream_t st);

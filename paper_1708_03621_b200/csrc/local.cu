@@ -245,10 +245,12 @@ int launch_cols_inv(const jdft_basis *b, const double2 *C, int nbt, double2 *W1,
     const int L = b->S[2];
     const size_t smem = 2 * (size_t)L * (kT + 1) * sizeof(double2);
     dim3 grid((b->ncol + kT - 1) / kT, nbt);
+    jdft_prof_begin(b, JDFT_K_COLS_INV, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         JDFT_CUDA(ensure_smem(k_cols_inv<LT>, smem));
         k_cols_inv<LT><<<grid, kNT, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
     });
+    jdft_prof_end(b, JDFT_K_COLS_INV, st);
     JDFT_LAUNCH_CHECK("k_cols_inv");
     return JDFT_OK;
 }
@@ -258,11 +260,13 @@ int launch_cols_fwd(const jdft_basis *b, const double2 *W1, int nbt, double scal
     const int L = b->S[2];
     const size_t smem = 2 * (size_t)L * (kT + 1) * sizeof(double2);
     dim3 grid((b->ncol + kT - 1) / kT, nbt);
+    jdft_prof_begin(b, JDFT_K_COLS_FWD, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         JDFT_CUDA(ensure_smem(k_cols_fwd<LT>, smem));
         k_cols_fwd<LT><<<grid, kNT, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
                                                 scale, kin, b->d_ke, C, out);
     });
+    jdft_prof_end(b, JDFT_K_COLS_FWD, st);
     JDFT_LAUNCH_CHECK("k_cols_fwd");
     return JDFT_OK;
 }
@@ -272,10 +276,12 @@ int launch_rows(const jdft_basis *b, int nbt, double2 *W1, double2 *W2, cudaStre
     const int L = b->S[1];
     const size_t smem = 2 * (size_t)L * kT * sizeof(double2) + (size_t)L * sizeof(int);
     dim3 grid((b->S[2] + kT - 1) / kT, b->npl, nbt);
+    jdft_prof_begin(b, FWD ? JDFT_K_ROWS_FWD : JDFT_K_ROWS_INV, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         JDFT_CUDA(ensure_smem(k_rows<LT, FWD>, smem));
         k_rows<LT, FWD><<<grid, kNT, smem, st>>>(b->plan[1], b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
     });
+    jdft_prof_end(b, FWD ? JDFT_K_ROWS_FWD : JDFT_K_ROWS_INV, st);
     JDFT_LAUNCH_CHECK("k_rows");
     return JDFT_OK;
 }
@@ -285,10 +291,12 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
     const int L = b->S[0];
     const size_t smem = 2 * (size_t)L * kT * sizeof(double2) + (size_t)L * sizeof(int);
     dim3 grid((b->S[2] + kT - 1) / kT, b->S[1], nbt);
+    jdft_prof_begin(b, JDFT_K_PLANES, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         JDFT_CUDA(ensure_smem(k_planes<LT, MODE>, smem));
         k_planes<LT, MODE><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V, psi);
     });
+    jdft_prof_end(b, JDFT_K_PLANES, st);
     JDFT_LAUNCH_CHECK("k_planes");
     return JDFT_OK;
 }
@@ -377,8 +385,10 @@ static int diag_op(const jdft_basis *b, const double *C, int nb, double *out, do
     if (total == 0) return JDFT_OK;
     int64_t blocks = (total + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
+    jdft_prof_begin(b, JDFT_K_DIAG, (cudaStream_t)s);
     k_diag<<<(int)blocks, 256, 0, (cudaStream_t)s>>>(b->nG, total, f0, f1, b->d_ke, reinterpret_cast<const double2 *>(C),
                                                       reinterpret_cast<double2 *>(out));
+    jdft_prof_end(b, JDFT_K_DIAG, (cudaStream_t)s);
     JDFT_LAUNCH_CHECK(who);
     return JDFT_OK;
 }

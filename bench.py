@@ -103,6 +103,22 @@ class ClockSampler:
         return out
 
 
+def max_over_ranks(x, world, device="cuda"):
+    """Max of a per-rank scalar over all ranks (the contract's max-over-ranks timing); identity for one rank."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(units_per_rank, world, ms_step_max):
+    """Whole-job throughput of N independent replicas: all ranks' units / the slowest rank's time."""
+    return world * units_per_rank / (ms_step_max * 1e-3)
+
+
 def config_sizes(cfg_id):
     cfg = workloads.get_config(cfg_id)
     return cfg, len(cfg["kpoints"]), cfg["nb"], cfg["natoms"] * cfg["n_lm"]
@@ -283,12 +299,9 @@ def run_ours(args):
         dom_n += n
         jd.jdft_set_option(k["gb"], "profile_kernel", 0)
     ms_step = float(np.mean(times))
-    if world > 1:
-        t = torch.tensor([ms_step], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step = float(t.item())
+    ms_step = max_over_ranks(ms_step, world)
     units = nb * nk
-    value = world * units / (ms_step * 1e-3)
+    value = aggregate_value(units, world, ms_step)
 
     # end to end through the HOST-buffer ABI call: pinned host inputs -> H2D -> kernels -> D2H, every step
     Vp = torch.from_numpy(Vh).pin_memory()
@@ -313,10 +326,7 @@ def run_ours(args):
         step_host()
     torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, world)
     h2d = sum(h["C"].numel() * 16 + h["P"].numel() * 16 + Vp.numel() * 8 + Dp.numel() * 8 +
               (2 * h["C"].numel() * 16 if do_overlap else 0) for h in host)
     d2h = sum(h["HC"].numel() * 16 + (h["M"].numel() * 16 if do_overlap else 0) for h in host)
@@ -364,7 +374,7 @@ def run_ours(args):
                    "nG": [k["gb"].nG for k in ks], "overlap_in_step": do_overlap, "l2": "flushed (512 MiB memset) before every timed step",
                    "parallelism": "replicas x%d" % world},
         "clocks": clocks,
-        "e2e": {"value": world * units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+        "e2e": {"value": aggregate_value(units, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms, "steps": e2e_steps},
         "gpu_launches": launches,
         "roofline": roofline,

@@ -53,7 +53,7 @@ def build(force=False, verbose=False):
             list(ex.map(run, jobs))
     if force or jobs or _stale(LIB, objs):
         tmp = LIB + ".tmp%d" % os.getpid()
-        run([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", tmp] + objs)  # static cudart (nvcc default)
+        run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-Wno-deprecated-gpu-targets", "-o", tmp] + objs)  # static cudart (nvcc default)
         os.replace(tmp, LIB)
     peak_src = os.path.join(CSRC, "fp64_peak.cu")
     if force or _stale(PEAK_TOOL, [peak_src]):

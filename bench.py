@@ -42,6 +42,19 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic(cfg_id, kernel):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full summary (profiles/traffic.csv), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        for line in f:
+            parts = line.strip().split(",")
+            if len(parts) >= 3 and parts[0] == str(cfg_id) and parts[1] == kernel:
+                return int(parts[2])
+    return None
+
+
 def fp64_peak():
     """Live DMMA / DFMA peak of this GPU from the committed micro-benchmark (csrc/fp64_peak.cu)."""
     tool = os.path.join(ROOT, "paper_1708_03621_b200", "fp64_peak")
@@ -356,11 +369,7 @@ def run_ours(args):
     roofline.update({"kernel": dominant, "launches_per_step": dom_n // args.steps,
                      "avg_launch_ms": dom_ms / max(1, dom_n), "peak_source": hbm_src if roofline["bound"] == "hbm" else fp_src,
                      "traffic": None, "share_of_step": dom_ms / args.steps / ms_step})
-    traffic_file = os.path.join(ROOT, "profiles", "traffic_r01.json")
-    if os.path.exists(traffic_file):
-        with open(traffic_file) as f:
-            tr = json.load(f)
-        roofline["traffic"] = tr.get("cfg%d" % args.config, {}).get(dominant)
+    roofline["traffic"] = ncu_traffic(args.config, dominant)
     local_bytes = sum(sum(algorithmic(k["info"], n, max(1, nbatches[n] // len(ks))) for n in
                           ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd")) for k in ks)
     local_ms = sum(per_kernel[n][0] for n in ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd"))

@@ -242,7 +242,7 @@ def run_ours(args):
         iG, _, _ = jd.jdft_basis_export(gb)
         C_h = workloads.make_bands(args.config, gb.nG, ik=ik)
         P_h = workloads.make_projectors(args.config, iG, kpts[ik], atoms)
-        jd.jdft_alloc_workspace(gb, max(args.batch, 16), max(nb, nproj))
+        jd.jdft_alloc_workspace(gb, max(args.batch, 64), max(nb, nproj))
         if args.batch > 0:
             jd.jdft_set_option(gb, "band_batch", args.batch)
         ks.append(dict(gb=gb, C=torch.from_numpy(C_h).cuda(), P=torch.from_numpy(P_h).cuda(),

@@ -336,11 +336,9 @@ int jdft_band_batch(const jdft_basis *b, int nb) {
     size_t fit = b->ws_bytes / per;
     int64_t want = b->opt_band_batch;
     if (want <= 0) {
-        // automatic: keep one batch's intermediates within ~half of the 126 MB L2 so the passes of a batch
-        // hand their data to each other through L2, but never fewer bands than fill the SMs once
-        const size_t target = (size_t)56 << 20;
-        want = (int64_t)(target / per);
-        if (want < 2) want = 2;
+        // automatic: as many bands as the workspace holds, up to 64.  Measured on B200 (profiles/r01_batch_sweep.md):
+        // filling the GPU (thousands of CTAs per launch, few tail waves) beats keeping a small batch L2-resident.
+        want = 64;
     }
     if ((size_t)want > fit) want = (int64_t)fit;
     if (want > nb) want = nb;

@@ -198,6 +198,164 @@ __global__ void __launch_bounds__(kNT) k_planes(const FftPlan plan, const double
     }
 }
 
+// ================================================================================================ tuned kernels
+// Two-pass specialised lengths (L = R1 R2: 32, 64, 72, 80, 128) run the kernels below instead of k_rows / k_planes<0>:
+//  * 16 pencils per CTA (256-byte global segments), thread count = 16 x (work items of the heaviest pass / 16) so
+//    that no thread idles at a barrier while others compute a butterfly;
+//  * ONE shared-memory tile [L][16] (half the footprint of the ping-pong engine -> twice the resident CTAs);
+//  * in k_planes_fused the inverse transform runs the radices (R1, R2) and the forward transform (R2, R1): the last
+//    inverse pass leaves a thread holding rows bf + R1 j (j < R2), which are exactly the inputs of the first forward
+//    pass, so IDFT_R2 -> * V_loc -> DFT_R2 happens in registers: 4 instead of 6 shared-memory tile transfers and
+//    3 instead of 4 barriers per pencil pair.
+template <int LT>
+struct Tuned {
+    static constexpr bool ok = SpecPlan<LT>::npass == 2;
+    static constexpr int R1 = SpecPlan<LT>::radix(0), R2 = SpecPlan<LT>::radix(1);
+    static constexpr int T = 16;
+    // threads = T x (butterflies of the pass that must run in one round = the R2 pass) rounded so the R1 pass is whole rounds
+    static constexpr int NB1 = ok ? LT / R1 : 1, NB2 = ok ? LT / R2 : 1;   // butterflies per pencil in the R1 / R2 pass
+    static constexpr int NBT = (NB1 % NB2 == 0) ? NB2 : (NB1 > NB2 ? NB1 : NB2);
+    static constexpr int NT = T * NBT;
+};
+
+template <int R, int SIGN>
+__device__ __forceinline__ void twiddle_rows(double2 (&a)[R], const double2 *__restrict__ tw, const int bf) {
+#pragma unroll
+    for (int j = 1; j < R; j++) {
+        double2 wv = __ldg(tw + bf * j);
+        if (SIGN < 0) wv.y = -wv.y;
+        a[j] = cmul(a[j], wv);
+    }
+}
+
+// K3 tuned: W2 -> IFFT axis 0 -> * V -> FFT axis 0 -> W2 (in place)
+template <int LT>
+__global__ void __launch_bounds__(Tuned<LT>::NT) k_planes_fused(const double2 *__restrict__ tw, const int S1, const int S2,
+                                                                const int npl, const int *__restrict__ planeof,
+                                                                double2 *__restrict__ W2, const double *__restrict__ V) {
+    using C = Tuned<LT>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, NT = C::NT, L = LT;
+    extern __shared__ double2 smem[];
+    double2 *A = smem;
+    __shared__ int s_planeof[L];
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y, b = blockIdx.z;
+    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    __syncthreads();
+    const size_t plane = (size_t)S1 * S2;
+    double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
+    const double *Vb = V + (size_t)i1 * S2 + t0;
+    const int tmax = S2 - t0;
+    // pass 0 of the inverse transform: radix R1, rows bf + k R2 -> rows bf R1 + j, twiddle w^(bf j)
+    for (int w = tid; w < R2 * T; w += NT) {
+        const int t = w % T, bf = w / T;
+        double2 a[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) {
+            const int p = s_planeof[bf + k * R2];
+            a[k] = (p >= 0 && t < tmax) ? W2b[p * plane + t] : make_double2(0.0, 0.0);
+        }
+        Dft<R1, +1>::run(a);
+        twiddle_rows<R1, +1>(a, tw, bf);
+#pragma unroll
+        for (int j = 0; j < R1; j++) A[(bf * R1 + j) * T + t] = a[j];
+    }
+    __syncthreads();
+    // last inverse pass (radix R2) -> * V -> first forward pass (radix R2), all in registers
+    {
+        static_assert(R1 * T <= NT, "the fused middle pass must run in one round");
+        const int t = tid % T, bf = tid / T;
+        const bool act = tid < R1 * T;
+        double2 a[R2];
+        if (act) {
+#pragma unroll
+            for (int k = 0; k < R2; k++) a[k] = A[(bf + k * R1) * T + t];
+        }
+        __syncthreads();
+        if (act) {
+            Dft<R2, +1>::run(a);
+#pragma unroll
+            for (int j = 0; j < R2; j++) {
+                const double f = t < tmax ? __ldg(Vb + (size_t)(bf + R1 * j) * plane + t) : 0.0;
+                a[j].x *= f;
+                a[j].y *= f;
+            }
+            Dft<R2, -1>::run(a);
+            twiddle_rows<R2, -1>(a, tw, bf);
+#pragma unroll
+            for (int j = 0; j < R2; j++) A[(bf * R2 + j) * T + t] = a[j];
+        }
+    }
+    __syncthreads();
+    // last forward pass: radix R1, rows bf + k R2 -> rows bf + R2 j (only the occupied planes are stored)
+    for (int w = tid; w < R2 * T; w += NT) {
+        const int t = w % T, bf = w / T;
+        double2 a[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) a[k] = A[(bf + k * R2) * T + t];
+        Dft<R1, -1>::run(a);
+#pragma unroll
+        for (int j = 0; j < R1; j++) {
+            const int p = s_planeof[bf + R2 * j];
+            if (p >= 0 && t < tmax) W2b[p * plane + t] = a[j];
+        }
+    }
+}
+
+// K2 / K4 tuned: one transform along axis 1 between compact columns (W1) and compact planes (W2)
+template <int LT, bool FWD>
+__global__ void __launch_bounds__(Tuned<LT>::NT) k_rows_tuned(const double2 *__restrict__ tw, const int S2, const int npl,
+                                                              const int ncol, const int *__restrict__ rowcol,
+                                                              double2 *__restrict__ W1, double2 *__restrict__ W2) {
+    using C = Tuned<LT>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, NT = C::NT, L = LT;
+    constexpr int SIGN = FWD ? -1 : +1;
+    extern __shared__ double2 smem[];
+    double2 *A = smem;
+    __shared__ int s_rowcol[L];
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, p = blockIdx.y, b = blockIdx.z;
+    for (int i = tid; i < L; i += NT) s_rowcol[i] = rowcol[p * L + i];
+    __syncthreads();
+    double2 *W1b = W1 + (size_t)b * ncol * S2 + t0;
+    double2 *W2b = W2 + ((size_t)b * npl + p) * L * S2 + t0;
+    const int tmax = S2 - t0;
+    for (int w = tid; w < R2 * T; w += NT) {
+        const int t = w % T, bf = w / T;
+        double2 a[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) {
+            const int row = bf + k * R2;
+            if (FWD) {
+                a[k] = t < tmax ? W2b[(size_t)row * S2 + t] : make_double2(0.0, 0.0);
+            } else {
+                const int c = s_rowcol[row];
+                a[k] = (c >= 0 && t < tmax) ? W1b[(size_t)c * S2 + t] : make_double2(0.0, 0.0);
+            }
+        }
+        Dft<R1, SIGN>::run(a);
+        twiddle_rows<R1, SIGN>(a, tw, bf);
+#pragma unroll
+        for (int j = 0; j < R1; j++) A[(bf * R1 + j) * T + t] = a[j];
+    }
+    __syncthreads();
+    for (int w = tid; w < R1 * T; w += NT) {
+        const int t = w % T, bf = w / T;
+        double2 a[R2];
+#pragma unroll
+        for (int k = 0; k < R2; k++) a[k] = A[(bf + k * R1) * T + t];
+        Dft<R2, SIGN>::run(a);
+#pragma unroll
+        for (int j = 0; j < R2; j++) {
+            const int row = bf + R1 * j;
+            if (FWD) {
+                const int c = s_rowcol[row];
+                if (c >= 0 && t < tmax) W1b[(size_t)c * S2 + t] = a[j];
+            } else {
+                if (t < tmax) W2b[(size_t)row * S2 + t] = a[j];
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ diagonal ops
 // out[b][n] = (f0 + f1 * ke[n]) * C[b][n]
 __global__ void k_diag(const int64_t nG, const int64_t total, const double f0, const double f1,
@@ -278,8 +436,16 @@ int launch_rows(const jdft_basis *b, int nbt, double2 *W1, double2 *W2, cudaStre
     dim3 grid((b->S[2] + kT - 1) / kT, b->npl, nbt);
     jdft_prof_begin(b, FWD ? JDFT_K_ROWS_FWD : JDFT_K_ROWS_INV, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
-        JDFT_CUDA(ensure_smem(k_rows<LT, FWD>, smem));
-        k_rows<LT, FWD><<<grid, kNT, smem, st>>>(b->plan[1], b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
+        if constexpr (Tuned<LT>::ok) {
+            using C = Tuned<LT>;
+            const size_t sm2 = (size_t)L * C::T * sizeof(double2);
+            JDFT_CUDA(ensure_smem(k_rows_tuned<LT, FWD>, sm2));
+            dim3 g2((b->S[2] + C::T - 1) / C::T, b->npl, nbt);
+            k_rows_tuned<LT, FWD><<<g2, C::NT, sm2, st>>>(b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
+        } else {
+            JDFT_CUDA(ensure_smem(k_rows<LT, FWD>, smem));
+            k_rows<LT, FWD><<<grid, kNT, smem, st>>>(b->plan[1], b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
+        }
     });
     jdft_prof_end(b, FWD ? JDFT_K_ROWS_FWD : JDFT_K_ROWS_INV, st);
     JDFT_LAUNCH_CHECK("k_rows");
@@ -293,8 +459,16 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
     dim3 grid((b->S[2] + kT - 1) / kT, b->S[1], nbt);
     jdft_prof_begin(b, JDFT_K_PLANES, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
-        JDFT_CUDA(ensure_smem(k_planes<LT, MODE>, smem));
-        k_planes<LT, MODE><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V, psi);
+        if constexpr (MODE == 0 && Tuned<LT>::ok) {
+            using C = Tuned<LT>;
+            const size_t sm2 = (size_t)L * C::T * sizeof(double2);
+            JDFT_CUDA(ensure_smem(k_planes_fused<LT>, sm2));
+            dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
+            k_planes_fused<LT><<<g2, C::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
+        } else {
+            JDFT_CUDA(ensure_smem(k_planes<LT, MODE>, smem));
+            k_planes<LT, MODE><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V, psi);
+        }
     });
     jdft_prof_end(b, JDFT_K_PLANES, st);
     JDFT_LAUNCH_CHECK("k_planes");

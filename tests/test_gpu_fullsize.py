@@ -24,10 +24,10 @@ def rel(got, want):
     return float(np.max(np.linalg.norm(got - want, axis=1) / np.linalg.norm(want, axis=1)))
 
 
-def auto_batch(gb, S):
-    """Bands per FFT batch the library picks on its own (W1 + W2 of a batch within ~56 MB)."""
+def auto_batch(gb, S, ws_bytes):
+    """Bands per FFT batch the library picks on its own (what the workspace holds, at most 64)."""
     per = 16 * (gb.ncol * S[2] + gb.npl * S[1] * S[2])
-    return max(2, (56 << 20) // per)
+    return max(1, min(64, ws_bytes // per))
 
 
 class Full:
@@ -42,8 +42,8 @@ class Full:
         inp = workloads.make_inputs(cfg_id, iG, ik=ik)
         self.C, self.V, self.P, self.D = inp["C"], inp["Vloc"], inp["P"], inp["D"]
         nproj = self.P.shape[0]
-        jd.jdft_alloc_workspace(self.gb, 16, max(self.nb, nproj))                          # as bench.py does
-        nbatch = auto_batch(self.gb, S)
+        ws = jd.jdft_alloc_workspace(self.gb, 64, max(self.nb, nproj))                     # as bench.py does
+        nbatch = auto_batch(self.gb, S, ws.numel())
         last0 = ((self.nb - 1) // nbatch) * nbatch                                         # first band of the last batch
         pick = {0, nbatch - 1, nbatch, last0, self.nb - 1}
         self.sample = sorted(b for b in pick if 0 <= b < self.nb)

@@ -250,11 +250,25 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     const int64_t ktiles = (K + BK - 1) / BK;
     const int tiles = ((Rn + BM - 1) / BM) * ((Cn + BN - 1) / BN);
     const size_t one = (size_t)Rn * Cn * 16;
-    int64_t nsplit = (148 * 3 + tiles - 1) / tiles;
-    if (nsplit > ktiles / 8) nsplit = ktiles / 8;
-    if (nsplit < 1) nsplit = 1;
-    if ((size_t)nsplit * one > scratch_bytes) nsplit = (int64_t)(scratch_bytes / one);
-    if (nsplit < 1) return jdft_fail(JDFT_EWORKSPACE, "gemm: workspace too small for a %d x %d result", Rn, Cn);
+    // Split K so that the grid fills whole waves of the 148 SMs x 2 resident CTAs (184 registers x 128 threads):
+    // among 1..6 waves take the first whose fill tiles*nsplit / (waves*slots) reaches 93 %, else the best one.
+    const int64_t slots = 148 * 2;
+    const int64_t max_by_k = ktiles / 16 > 0 ? ktiles / 16 : 1;              // at least 16 k-tiles (128 k) per slice
+    const int64_t max_by_ws = (int64_t)(scratch_bytes / one);
+    if (max_by_ws < 1) return jdft_fail(JDFT_EWORKSPACE, "gemm: workspace too small for a %d x %d result", Rn, Cn);
+    int64_t nsplit = 1;
+    double best = -1.0;
+    for (int64_t w = 1; w <= 6; w++) {
+        int64_t ns = (w * slots) / tiles;
+        if (ns > max_by_k) ns = max_by_k;
+        if (ns > max_by_ws) ns = max_by_ws;
+        if (ns < 1) ns = 1;
+        const int64_t ctas = ns * tiles;
+        const int64_t waves = (ctas + slots - 1) / slots;
+        const double fill = (double)ctas / (double)(waves * slots);
+        if (fill > best + 1e-9) { best = fill; nsplit = ns; }
+        if (best >= 0.93) break;
+    }
     int64_t per = (ktiles + nsplit - 1) / nsplit;
     if (per < 1) per = 1;
     nsplit = (ktiles + per - 1) / per;

@@ -14,6 +14,10 @@ namespace {
 
 constexpr int kT = 8;      // pencils per CTA
 constexpr int kNT = 128;   // threads per CTA
+// threads per CTA of the column kernels: the work items of a pass, (L / radix) x kT, should be whole rounds
+template <int LT> struct ColsNT { static constexpr int v = kNT; };
+template <> struct ColsNT<216> { static constexpr int v = 288; };   // 6 x 6 x 6: 36 x 8 items in every pass
+template <> struct ColsNT<32> { static constexpr int v = 64; };     // 4 x 8: 64 and 32 items
 
 __device__ __forceinline__ int wrapi(int m, int S) {
     int r = m % S;
@@ -22,11 +26,11 @@ __device__ __forceinline__ int wrapi(int m, int S) {
 
 // ------------------------------------------------------------------------------------------------ K1
 template <int LT>
-__global__ void __launch_bounds__(kNT) k_cols_inv(const FftPlan plan, const double2 *__restrict__ tw, const int ncol,
+__global__ void __launch_bounds__(ColsNT<LT>::v) k_cols_inv(const FftPlan plan, const double2 *__restrict__ tw, const int ncol,
                                                   const int64_t nG, const int *__restrict__ col_n0,
                                                   const int *__restrict__ col_m2lo, const double2 *__restrict__ C,
                                                   double2 *__restrict__ W1) {
-    constexpr int T = kT, TP = kT + 1, NT = kNT;
+    constexpr int T = kT, TP = kT + 1, NT = ColsNT<LT>::v;
     const int L = LT > 0 ? LT : plan.L;
     extern __shared__ double2 smem[];
     double2 *bufA = smem, *bufB = smem + L * TP;
@@ -62,12 +66,12 @@ __global__ void __launch_bounds__(kNT) k_cols_inv(const FftPlan plan, const doub
 // ------------------------------------------------------------------------------------------------ K5
 // out[b][n] = scale * (F_2 W1)[column of n][m2 of n]  (+ kin * ke[n] * C[b][n])
 template <int LT>
-__global__ void __launch_bounds__(kNT) k_cols_fwd(const FftPlan plan, const double2 *__restrict__ tw, const int ncol,
+__global__ void __launch_bounds__(ColsNT<LT>::v) k_cols_fwd(const FftPlan plan, const double2 *__restrict__ tw, const int ncol,
                                                   const int64_t nG, const int *__restrict__ col_n0,
                                                   const int *__restrict__ col_m2lo, const double2 *__restrict__ W1,
                                                   const double scale, const double kin, const double *__restrict__ ke,
                                                   const double2 *__restrict__ C, double2 *__restrict__ outC) {
-    constexpr int T = kT, TP = kT + 1, NT = kNT;
+    constexpr int T = kT, TP = kT + 1, NT = ColsNT<LT>::v;
     const int L = LT > 0 ? LT : plan.L;
     extern __shared__ double2 smem[];
     double2 *bufA = smem, *bufB = smem + L * TP;
@@ -228,9 +232,16 @@ __device__ __forceinline__ void twiddle_rows(double2 (&a)[R], const double2 *__r
     }
 }
 
+// resident CTAs per SM the register allocation of k_planes_fused is bounded for (measured: profiles/r01_planes_tuning.md)
+template <int LT> struct PlanesMinB { static constexpr int v = 4; };
+#ifndef PLANES_MINB_80
+#define PLANES_MINB_80 5
+#endif
+template <> struct PlanesMinB<80> { static constexpr int v = PLANES_MINB_80; };
+template <> struct PlanesMinB<72> { static constexpr int v = 6; };
 // K3 tuned: W2 -> IFFT axis 0 -> * V -> FFT axis 0 -> W2 (in place)
 template <int LT>
-__global__ void __launch_bounds__(Tuned<LT>::NT) k_planes_fused(const double2 *__restrict__ tw, const int S1, const int S2,
+__global__ void __launch_bounds__(Tuned<LT>::NT, PlanesMinB<LT>::v) k_planes_fused(const double2 *__restrict__ tw, const int S1, const int S2,
                                                                 const int npl, const int *__restrict__ planeof,
                                                                 double2 *__restrict__ W2, const double *__restrict__ V) {
     using C = Tuned<LT>;
@@ -406,7 +417,7 @@ int launch_cols_inv(const jdft_basis *b, const double2 *C, int nbt, double2 *W1,
     jdft_prof_begin(b, JDFT_K_COLS_INV, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         JDFT_CUDA(ensure_smem(k_cols_inv<LT>, smem));
-        k_cols_inv<LT><<<grid, kNT, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+        k_cols_inv<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
     });
     jdft_prof_end(b, JDFT_K_COLS_INV, st);
     JDFT_LAUNCH_CHECK("k_cols_inv");
@@ -421,7 +432,7 @@ int launch_cols_fwd(const jdft_basis *b, const double2 *W1, int nbt, double scal
     jdft_prof_begin(b, JDFT_K_COLS_FWD, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         JDFT_CUDA(ensure_smem(k_cols_fwd<LT>, smem));
-        k_cols_fwd<LT><<<grid, kNT, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
+        k_cols_fwd<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
                                                 scale, kin, b->d_ke, C, out);
     });
     jdft_prof_end(b, JDFT_K_COLS_FWD, st);

@@ -1,0 +1,271 @@
+// Tuned column kernels (K1: scatter + inverse FFT along axis 2; K5: forward FFT along axis 2 + gather + kinetic)
+// for the lengths that have compile-time plans (fft.cuh SpecPlan).  Included by local.cu only.
+//
+// Both kernels are bound by shared-memory bandwidth, not HBM (profiles/r01_ncu_full_cfg2_fft.md), so the design
+// goal is fewer shared-memory tile transfers than the ping-pong engine needs:
+//   K1  no zero fill (the first pass tests "is this row inside the column's sphere run" instead), and the last pass
+//       writes W1 straight from registers with the lanes of a warp running along the pencil (consecutive rows ->
+//       128..512-byte global segments), so there is no transposition through shared memory;
+//   K5  the first pass reads W1 straight from global memory the same way (lanes along the pencil) and writes its
+//       butterflies into an XOR-swizzled tile, so the load staging disappears as well.
+// Tiles are [L][TP] c128 with TP = T + 1 (T pencils per CTA); the swizzled tile uses stride T inside the same buffer.
+#pragma once
+#include "fft.cuh"
+
+namespace jcols {
+using namespace jfft;
+
+template <int LT>
+struct Cfg {
+    using P = SpecPlan<LT>;
+    static constexpr int NP = P::npass;
+    static constexpr bool ok = NP == 2 || NP == 3;
+    static constexpr int R0 = P::r0, R1 = P::r1, R2 = P::r2;
+    static constexpr int RL = NP == 3 ? R2 : R1;               // radix of the last pass
+    static constexpr int T = NP == 3 ? 8 : 16;                  // pencils per CTA
+    static constexpr int TP = T + 1;
+    static constexpr int NBL = ok ? LT / RL : 1;                // butterflies per pencil in the last pass
+    static constexpr int NB0 = ok ? LT / R0 : 1;                // ... in the first pass
+    // two-pass plans: ONE swizzled tile [L][T], first pass in a single round (threads = its work items);
+    // three-pass plans: two padded tiles [L][TP]
+    static constexpr int NT = NP == 3 ? T * (NB0 % NBL == 0 ? NBL : (NB0 > NBL ? NB0 : NBL)) : T * NB0;
+    static constexpr size_t smem = NP == 3 ? 2 * (size_t)LT * TP * sizeof(double2) : (size_t)LT * T * sizeof(double2);
+    // swizzled position of (row, pencil t): conflict-free for lanes along t, along butterflies and along rows
+    static __device__ __forceinline__ int sw(int row, int t) { return row * T + (t ^ ((row + row / R0) & (T - 1))); }
+};
+
+__device__ __forceinline__ int wrap_row(int m, int L) {
+    int r = m % L;
+    return r < 0 ? r + L : r;
+}
+
+template <int R, int SIGN>
+__device__ __forceinline__ void tw_mul(double2 (&a)[R], const double2 *__restrict__ tw, const int pb) {
+#pragma unroll
+    for (int j = 1; j < R; j++) {
+        double2 wv = __ldg(tw + pb * j);
+        if (SIGN < 0) wv.y = -wv.y;
+        a[j] = cmul(a[j], wv);
+    }
+}
+
+// middle pass of a three-pass plan, shared -> shared, pencil index fastest: radix R, s = product of earlier radices
+template <int LT, int R, int SIGN, int T, int NT, class Ld, class St>
+__device__ __forceinline__ void mid_pass(const int s, const double2 *__restrict__ tw, Ld ld, St st) {
+    constexpr int nbf = LT / R;
+    for (int w = threadIdx.x; w < nbf * T; w += NT) {
+        const int t = w % T, bf = w / T;
+        double2 a[R];
+#pragma unroll
+        for (int k = 0; k < R; k++) a[k] = ld(bf + k * nbf, t);
+        Dft<R, SIGN>::run(a);
+        const int q = bf % s, pb = bf - q;
+        tw_mul<R, SIGN>(a, tw, pb);
+#pragma unroll
+        for (int j = 0; j < R; j++) st(q + pb * R + s * j, t, a[j]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K1
+template <int LT>
+__global__ void __launch_bounds__(Cfg<LT>::NT) k_cols_inv_tuned(const double2 *__restrict__ tw, const int ncol,
+                                                                const int64_t nG, const int *__restrict__ col_n0,
+                                                                const int *__restrict__ col_m2lo,
+                                                                const double2 *__restrict__ C, double2 *__restrict__ W1) {
+    using F = Cfg<LT>;
+    constexpr int T = F::T, TP = F::TP, NT = F::NT, L = LT, R0 = F::R0, R1 = F::R1, RL = F::RL, NBL = F::NBL, NB0 = F::NB0;
+    extern __shared__ double2 smem[];
+    double2 *X = smem, *Y = smem + L * TP;
+    __shared__ int s_n0[T + 1], s_m2w[T];
+    const int tid = threadIdx.x, c0 = blockIdx.x * T, b = blockIdx.y;
+    const int nc = min(T, ncol - c0);
+    if (tid <= T) s_n0[tid] = col_n0[min(c0 + tid, ncol)];
+    if (tid < T) s_m2w[tid] = wrap_row(col_m2lo[min(c0 + tid, ncol - 1)], L);
+    __syncthreads();
+    const double2 *Cb = C + (size_t)b * nG;
+    double2 *Wb = W1 + ((size_t)b * ncol + c0) * L;
+    const int nbeg = s_n0[0], nend = s_n0[nc];
+    if constexpr (F::NP == 2) {
+        // scatter the sphere runs of the nc columns (contiguous in n) into the tile; nothing else of it is read
+        for (int e = tid; e < nend - nbeg; e += NT) {
+            const int n = nbeg + e;
+            int t = 0;
+            while (n >= s_n0[t + 1]) t++;
+            int row = s_m2w[t] + (n - s_n0[t]);
+            if (row >= L) row -= L;
+            X[F::sw(row, t)] = Cb[n];
+        }
+        __syncthreads();
+        // pass 0 (radix R0, s = 1), one round, in place: rows bf + k NB0 (zero outside the run) -> rows bf R0 + j
+        {
+            const int t = tid % T, bf = tid / T;
+            const int m2w = s_m2w[t], len = t < nc ? s_n0[t + 1] - s_n0[t] : 0;
+            double2 a[R0];
+#pragma unroll
+            for (int k = 0; k < R0; k++) {
+                const int row = bf + k * NB0;
+                int off = row - m2w;
+                if (off < 0) off += L;
+                a[k] = make_double2(0.0, 0.0);
+                if (off < len) a[k] = X[F::sw(row, t)];
+            }
+            __syncthreads();
+            Dft<R0, +1>::run(a);
+            tw_mul<R0, +1>(a, tw, bf);
+#pragma unroll
+            for (int j = 0; j < R0; j++) X[F::sw(bf * R0 + j, t)] = a[j];
+        }
+        __syncthreads();
+        // last pass (radix R1): lanes run along the pencil, outputs go straight to W1[column][row]
+        for (int w = tid; w < NBL * T; w += NT) {
+            const int bf = w % NBL, t = w / NBL;
+            double2 a[RL];
+#pragma unroll
+            for (int k = 0; k < RL; k++) a[k] = X[F::sw(bf + k * NBL, t)];
+            Dft<RL, +1>::run(a);
+            if (t < nc) {
+#pragma unroll
+                for (int j = 0; j < RL; j++) Wb[(size_t)t * L + bf + NBL * j] = a[j];
+            }
+        }
+    } else {
+        for (int e = tid; e < nend - nbeg; e += NT) {
+            const int n = nbeg + e;
+            int t = 0;
+            while (n >= s_n0[t + 1]) t++;
+            int row = s_m2w[t] + (n - s_n0[t]);
+            if (row >= L) row -= L;
+            X[row * TP + t] = Cb[n];
+        }
+        __syncthreads();
+        for (int w = tid; w < NB0 * T; w += NT) {
+            const int t = w % T, bf = w / T;
+            const int m2w = s_m2w[t], len = t < nc ? s_n0[t + 1] - s_n0[t] : 0;
+            double2 a[R0];
+#pragma unroll
+            for (int k = 0; k < R0; k++) {
+                const int row = bf + k * NB0;
+                int off = row - m2w;
+                if (off < 0) off += L;
+                a[k] = make_double2(0.0, 0.0);
+                if (off < len) a[k] = X[row * TP + t];
+            }
+            Dft<R0, +1>::run(a);
+            tw_mul<R0, +1>(a, tw, bf);
+#pragma unroll
+            for (int j = 0; j < R0; j++) Y[(bf * R0 + j) * TP + t] = a[j];
+        }
+        __syncthreads();
+        mid_pass<LT, R1, +1, T, NT>(
+            R0, tw, [&](int row, int t) { return Y[row * TP + t]; },
+            [&](int row, int t, double2 v) { X[row * TP + t] = v; });
+        __syncthreads();
+        for (int w = tid; w < NBL * T; w += NT) {
+            const int bf = w % NBL, t = w / NBL;
+            double2 a[RL];
+#pragma unroll
+            for (int k = 0; k < RL; k++) a[k] = X[(bf + k * NBL) * TP + t];
+            Dft<RL, +1>::run(a);
+            if (t < nc) {
+#pragma unroll
+                for (int j = 0; j < RL; j++) Wb[(size_t)t * L + bf + NBL * j] = a[j];
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K5
+// out[b][n] = scale * (F_2 W1)[column of n][m2 of n]  (+ kin * ke[n] * C[b][n])
+template <int LT>
+__global__ void __launch_bounds__(Cfg<LT>::NT) k_cols_fwd_tuned(const double2 *__restrict__ tw, const int ncol,
+                                                                const int64_t nG, const int *__restrict__ col_n0,
+                                                                const int *__restrict__ col_m2lo,
+                                                                const double2 *__restrict__ W1, const double scale,
+                                                                const double kin, const double *__restrict__ ke,
+                                                                const double2 *__restrict__ C, double2 *__restrict__ outC) {
+    using F = Cfg<LT>;
+    constexpr int T = F::T, TP = F::TP, NT = F::NT, L = LT, R0 = F::R0, R1 = F::R1, RL = F::RL, NBL = F::NBL, NB0 = F::NB0;
+    extern __shared__ double2 smem[];
+    double2 *X = smem, *Y = smem + L * TP;
+    __shared__ int s_n0[T + 1], s_m2w[T];
+    const int tid = threadIdx.x, c0 = blockIdx.x * T, b = blockIdx.y;
+    const int nc = min(T, ncol - c0);
+    if (tid <= T) s_n0[tid] = col_n0[min(c0 + tid, ncol)];
+    if (tid < T) s_m2w[tid] = wrap_row(col_m2lo[min(c0 + tid, ncol - 1)], L);
+    // pass 0 (radix R0, s = 1): lanes run along the pencil, inputs straight from W1[column][row]
+    const double2 *Wb = W1 + ((size_t)b * ncol + c0) * L;
+    if constexpr (F::NP == 2) {
+        for (int w = tid; w < NB0 * T; w += NT) {
+            const int bf = w % NB0, t = w / NB0;
+            double2 a[R0];
+#pragma unroll
+            for (int k = 0; k < R0; k++) a[k] = t < nc ? Wb[(size_t)t * L + bf + k * NB0] : make_double2(0.0, 0.0);
+            Dft<R0, -1>::run(a);
+            tw_mul<R0, -1>(a, tw, bf);
+#pragma unroll
+            for (int j = 0; j < R0; j++) X[F::sw(bf * R0 + j, t)] = a[j];
+        }
+        __syncthreads();
+        // last pass (radix R1), in place: a thread reads and writes the same rows bf + NBL k of its pencil
+        for (int w = tid; w < NBL * T; w += NT) {
+            const int t = w % T, bf = w / T;
+            double2 a[RL];
+#pragma unroll
+            for (int k = 0; k < RL; k++) a[k] = X[F::sw(bf + k * NBL, t)];
+            Dft<RL, -1>::run(a);
+#pragma unroll
+            for (int j = 0; j < RL; j++) X[F::sw(bf + NBL * j, t)] = a[j];
+        }
+    } else {
+        // outputs to the XOR-swizzled tile X[row][t ^ ((row / R0) % T)] (conflict-free for this pass and the next)
+        for (int w = tid; w < NB0 * T; w += NT) {
+            const int bf = w % NB0, t = w / NB0;
+            double2 a[R0];
+#pragma unroll
+            for (int k = 0; k < R0; k++) a[k] = t < nc ? Wb[(size_t)t * L + bf + k * NB0] : make_double2(0.0, 0.0);
+            Dft<R0, -1>::run(a);
+            tw_mul<R0, -1>(a, tw, bf);
+            const int tx = t ^ (bf % T);
+#pragma unroll
+            for (int j = 0; j < R0; j++) X[(bf * R0 + j) * T + tx] = a[j];
+        }
+        __syncthreads();
+        mid_pass<LT, R1, -1, T, NT>(
+            R0, tw, [&](int row, int t) { return X[row * T + (t ^ ((row / R0) % T))]; },
+            [&](int row, int t, double2 v) { Y[row * TP + t] = v; });
+        __syncthreads();
+        for (int w = tid; w < NBL * T; w += NT) {
+            const int t = w % T, bf = w / T;
+            double2 a[RL];
+#pragma unroll
+            for (int k = 0; k < RL; k++) a[k] = Y[(bf + k * NBL) * TP + t];
+            Dft<RL, -1>::run(a);
+#pragma unroll
+            for (int j = 0; j < RL; j++) X[(bf + NBL * j) * TP + t] = a[j];
+        }
+    }
+    __syncthreads();
+    // gather the sphere runs (contiguous in n) and add the kinetic term
+    const int nbeg = s_n0[0], nend = s_n0[nc];
+    const double2 *Cb = C + (size_t)b * nG;
+    double2 *Ob = outC + (size_t)b * nG;
+    for (int e = tid; e < nend - nbeg; e += NT) {
+        const int n = nbeg + e;
+        int t = 0;
+        while (n >= s_n0[t + 1]) t++;
+        int row = s_m2w[t] + (n - s_n0[t]);
+        if (row >= L) row -= L;
+        double2 v = F::NP == 2 ? X[F::sw(row, t)] : X[row * TP + t];
+        v.x *= scale;
+        v.y *= scale;
+        if (kin != 0.0) {
+            const double f = kin * ke[n];
+            const double2 c = Cb[n];
+            v.x = fma(f, c.x, v.x);
+            v.y = fma(f, c.y, v.y);
+        }
+        Ob[n] = v;
+    }
+}
+
+}  // namespace jcols

@@ -197,18 +197,21 @@ JFFT_COMPOSITE(16, 4, 4)
 template <int L>
 struct SpecPlan {
     static constexpr int npass = 0;  // no specialisation
+    static constexpr int r0 = 1, r1 = 1, r2 = 1;
     static constexpr int radix(int) { return 1; }
 };
 #define JFFT_SPEC2(L, A, B)                                                 \
     template <>                                                              \
     struct SpecPlan<L> {                                                     \
         static constexpr int npass = 2;                                      \
+        static constexpr int r0 = A, r1 = B, r2 = 1;                         \
         static constexpr int radix(int i) { return i == 0 ? A : B; }         \
     };
 #define JFFT_SPEC3(L, A, B, C)                                               \
     template <>                                                              \
     struct SpecPlan<L> {                                                     \
         static constexpr int npass = 3;                                      \
+        static constexpr int r0 = A, r1 = B, r2 = C;                         \
         static constexpr int radix(int i) { return i == 0 ? A : (i == 1 ? B : C); } \
     };
 JFFT_SPEC2(32, 4, 8)

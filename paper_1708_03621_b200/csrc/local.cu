@@ -7,6 +7,7 @@
 //   K5 k_cols_fwd   forward FFT along axis 2 (+) gather box -> sphere (+) + Omega ke C   (the -1/2 L C term)
 // Intermediates: W1 [nbatch][ncol][S2] and W2 [nbatch][npl][S1][S2] (c128) in the caller's workspace.
 #include "fft.cuh"
+#include "cols_tuned.cuh"
 
 using namespace jfft;
 
@@ -416,8 +417,15 @@ int launch_cols_inv(const jdft_basis *b, const double2 *C, int nbt, double2 *W1,
     dim3 grid((b->ncol + kT - 1) / kT, nbt);
     jdft_prof_begin(b, JDFT_K_COLS_INV, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
-        JDFT_CUDA(ensure_smem(k_cols_inv<LT>, smem));
-        k_cols_inv<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+        if constexpr (jcols::Cfg<LT>::ok) {
+            using F = jcols::Cfg<LT>;
+            JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT>, F::smem));
+            dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
+            jcols::k_cols_inv_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+        } else {
+            JDFT_CUDA(ensure_smem(k_cols_inv<LT>, smem));
+            k_cols_inv<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+        }
     });
     jdft_prof_end(b, JDFT_K_COLS_INV, st);
     JDFT_LAUNCH_CHECK("k_cols_inv");
@@ -431,9 +439,17 @@ int launch_cols_fwd(const jdft_basis *b, const double2 *W1, int nbt, double scal
     dim3 grid((b->ncol + kT - 1) / kT, nbt);
     jdft_prof_begin(b, JDFT_K_COLS_FWD, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
-        JDFT_CUDA(ensure_smem(k_cols_fwd<LT>, smem));
-        k_cols_fwd<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
-                                                scale, kin, b->d_ke, C, out);
+        if constexpr (jcols::Cfg<LT>::ok) {
+            using F = jcols::Cfg<LT>;
+            JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT>, F::smem));
+            dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
+            jcols::k_cols_fwd_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
+                                                               scale, kin, b->d_ke, C, out);
+        } else {
+            JDFT_CUDA(ensure_smem(k_cols_fwd<LT>, smem));
+            k_cols_fwd<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
+                                                    scale, kin, b->d_ke, C, out);
+    }
     });
     jdft_prof_end(b, JDFT_K_COLS_FWD, st);
     JDFT_LAUNCH_CHECK("k_cols_fwd");

@@ -28,10 +28,12 @@ struct Cfg {
     static constexpr int MINB = (LT == 128 || LT == 216) ? 4 : 6;
     static constexpr int NBL = ok ? LT / RL : 1;                // butterflies per pencil in the last pass
     static constexpr int NB0 = ok ? LT / R0 : 1;                // ... in the first pass
-    // two-pass plans: ONE swizzled tile [L][T], first pass in a single round (threads = its work items);
-    // three-pass plans: two padded tiles [L][TP]
-    static constexpr int NT = NP == 3 ? T * (NB0 % NBL == 0 ? NBL : (NB0 > NBL ? NB0 : NBL)) : T * NB0;
-    static constexpr size_t smem = NP == 3 ? 2 * (size_t)LT * TP * sizeof(double2) : (size_t)LT * T * sizeof(double2);
+    // ONE swizzled tile [L][T]; the shared -> shared passes run in a single round (threads = their work items) and
+    // in place: every thread reads its butterfly, barrier, writes it back
+    static constexpr int NT = T * NB0;
+    static constexpr int NB1 = ok ? LT / R1 : 1;                // butterflies per pencil in the middle pass (3-pass plans)
+    static_assert(NP != 3 || NB1 * T == NT, "middle pass must be exactly one round");
+    static constexpr size_t smem = (size_t)LT * T * sizeof(double2);
     // swizzled position of (row, pencil t): conflict-free for lanes along t, along butterflies and along rows
     static __device__ __forceinline__ int sw(int row, int t) { return row * T + (t ^ ((row + row / R0) & (T - 1))); }
 };
@@ -39,6 +41,16 @@ struct Cfg {
 __device__ __forceinline__ int wrap_row(int m, int L) {
     int r = m % L;
     return r < 0 ? r + L : r;
+}
+
+// column t of sphere entry n among the CTA's T columns: largest t with s_n0[t] <= n (branch-free binary search)
+template <int T>
+__device__ __forceinline__ int find_col(const int *s_n0, const int n) {
+    int t = 0;
+#pragma unroll
+    for (int h = T / 2; h >= 1; h >>= 1)
+        if (n >= s_n0[t + h]) t += h;
+    return t;
 }
 
 template <int R, int SIGN>
@@ -51,21 +63,23 @@ __device__ __forceinline__ void tw_mul(double2 (&a)[R], const double2 *__restric
     }
 }
 
-// middle pass of a three-pass plan, shared -> shared, pencil index fastest: radix R, s = product of earlier radices
-template <int LT, int R, int SIGN, int T, int NT, class Ld, class St>
-__device__ __forceinline__ void mid_pass(const int s, const double2 *__restrict__ tw, Ld ld, St st) {
-    constexpr int nbf = LT / R;
-    for (int w = threadIdx.x; w < nbf * T; w += NT) {
-        const int t = w % T, bf = w / T;
-        double2 a[R];
+// middle pass of a three-pass plan, in place in the swizzled tile, one round, pencil index fastest:
+// radix R1, s = R0 (Stockham: rows bf + k NB1 -> rows q + pb R1 + s j, twiddle w^(pb j), q = bf mod s, pb = bf - q)
+template <int LT, int SIGN>
+__device__ __forceinline__ void mid_pass_inplace(double2 *X, const double2 *__restrict__ tw) {
+    using F = Cfg<LT>;
+    constexpr int R = F::R1, nbf = F::NB1, s = F::R0, T = F::T;
+    const int t = threadIdx.x % T, bf = threadIdx.x / T;
+    double2 a[R];
 #pragma unroll
-        for (int k = 0; k < R; k++) a[k] = ld(bf + k * nbf, t);
-        Dft<R, SIGN>::run(a);
-        const int q = bf % s, pb = bf - q;
-        tw_mul<R, SIGN>(a, tw, pb);
+    for (int k = 0; k < R; k++) a[k] = X[F::sw(bf + k * nbf, t)];
+    __syncthreads();
+    Dft<R, SIGN>::run(a);
+    const int q = bf % s, pb = bf - q;
+    tw_mul<R, SIGN>(a, tw, pb);
 #pragma unroll
-        for (int j = 0; j < R; j++) st(q + pb * R + s * j, t, a[j]);
-    }
+    for (int j = 0; j < R; j++) X[F::sw(q + pb * R + s * j, t)] = a[j];
+    __syncthreads();
 }
 
 // ------------------------------------------------------------------------------------------------ K1
@@ -77,7 +91,7 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_inv_tuned(c
     using F = Cfg<LT>;
     constexpr int T = F::T, TP = F::TP, NT = F::NT, L = LT, R0 = F::R0, R1 = F::R1, RL = F::RL, NBL = F::NBL, NB0 = F::NB0;
     extern __shared__ double2 smem[];
-    double2 *X = smem, *Y = smem + L * TP;
+    double2 *X = smem;
     __shared__ int s_n0[T + 1], s_m2w[T];
     const int tid = threadIdx.x, c0 = blockIdx.x * T, b = blockIdx.y;
     const int nc = min(T, ncol - c0);
@@ -87,12 +101,11 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_inv_tuned(c
     const double2 *Cb = C + (size_t)b * nG;
     double2 *Wb = W1 + ((size_t)b * ncol + c0) * L;
     const int nbeg = s_n0[0], nend = s_n0[nc];
-    if constexpr (F::NP == 2) {
+    {
         // scatter the sphere runs of the nc columns (contiguous in n) into the tile; nothing else of it is read
         for (int e = tid; e < nend - nbeg; e += NT) {
             const int n = nbeg + e;
-            int t = 0;
-            while (n >= s_n0[t + 1]) t++;
+            const int t = find_col<T>(s_n0, n);
             int row = s_m2w[t] + (n - s_n0[t]);
             if (row >= L) row -= L;
             X[F::sw(row, t)] = Cb[n];
@@ -118,55 +131,13 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_inv_tuned(c
             for (int j = 0; j < R0; j++) X[F::sw(bf * R0 + j, t)] = a[j];
         }
         __syncthreads();
-        // last pass (radix R1): lanes run along the pencil, outputs go straight to W1[column][row]
+        if constexpr (F::NP == 3) mid_pass_inplace<LT, +1>(X, tw);
+        // last pass (radix RL): lanes run along the pencil, outputs go straight to W1[column][row]
         for (int w = tid; w < NBL * T; w += NT) {
             const int bf = w % NBL, t = w / NBL;
             double2 a[RL];
 #pragma unroll
             for (int k = 0; k < RL; k++) a[k] = X[F::sw(bf + k * NBL, t)];
-            Dft<RL, +1>::run(a);
-            if (t < nc) {
-#pragma unroll
-                for (int j = 0; j < RL; j++) Wb[(size_t)t * L + bf + NBL * j] = a[j];
-            }
-        }
-    } else {
-        for (int e = tid; e < nend - nbeg; e += NT) {
-            const int n = nbeg + e;
-            int t = 0;
-            while (n >= s_n0[t + 1]) t++;
-            int row = s_m2w[t] + (n - s_n0[t]);
-            if (row >= L) row -= L;
-            X[row * TP + t] = Cb[n];
-        }
-        __syncthreads();
-        for (int w = tid; w < NB0 * T; w += NT) {
-            const int t = w % T, bf = w / T;
-            const int m2w = s_m2w[t], len = t < nc ? s_n0[t + 1] - s_n0[t] : 0;
-            double2 a[R0];
-#pragma unroll
-            for (int k = 0; k < R0; k++) {
-                const int row = bf + k * NB0;
-                int off = row - m2w;
-                if (off < 0) off += L;
-                a[k] = make_double2(0.0, 0.0);
-                if (off < len) a[k] = X[row * TP + t];
-            }
-            Dft<R0, +1>::run(a);
-            tw_mul<R0, +1>(a, tw, bf);
-#pragma unroll
-            for (int j = 0; j < R0; j++) Y[(bf * R0 + j) * TP + t] = a[j];
-        }
-        __syncthreads();
-        mid_pass<LT, R1, +1, T, NT>(
-            R0, tw, [&](int row, int t) { return Y[row * TP + t]; },
-            [&](int row, int t, double2 v) { X[row * TP + t] = v; });
-        __syncthreads();
-        for (int w = tid; w < NBL * T; w += NT) {
-            const int bf = w % NBL, t = w / NBL;
-            double2 a[RL];
-#pragma unroll
-            for (int k = 0; k < RL; k++) a[k] = X[(bf + k * NBL) * TP + t];
             Dft<RL, +1>::run(a);
             if (t < nc) {
 #pragma unroll
@@ -188,7 +159,7 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_fwd_tuned(c
     using F = Cfg<LT>;
     constexpr int T = F::T, TP = F::TP, NT = F::NT, L = LT, R0 = F::R0, R1 = F::R1, RL = F::RL, NBL = F::NBL, NB0 = F::NB0;
     extern __shared__ double2 smem[];
-    double2 *X = smem, *Y = smem + L * TP;
+    double2 *X = smem;
     __shared__ int s_n0[T + 1], s_m2w[T];
     const int tid = threadIdx.x, c0 = blockIdx.x * T, b = blockIdx.y;
     const int nc = min(T, ncol - c0);
@@ -196,7 +167,7 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_fwd_tuned(c
     if (tid < T) s_m2w[tid] = wrap_row(col_m2lo[min(c0 + tid, ncol - 1)], L);
     // pass 0 (radix R0, s = 1): lanes run along the pencil, inputs straight from W1[column][row]
     const double2 *Wb = W1 + ((size_t)b * ncol + c0) * L;
-    if constexpr (F::NP == 2) {
+    {
         for (int w = tid; w < NB0 * T; w += NT) {
             const int bf = w % NB0, t = w / NB0;
             double2 a[R0];
@@ -208,7 +179,8 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_fwd_tuned(c
             for (int j = 0; j < R0; j++) X[F::sw(bf * R0 + j, t)] = a[j];
         }
         __syncthreads();
-        // last pass (radix R1), in place: a thread reads and writes the same rows bf + NBL k of its pencil
+        if constexpr (F::NP == 3) mid_pass_inplace<LT, -1>(X, tw);
+        // last pass (radix RL), in place: a thread reads and writes the same rows bf + NBL k of its pencil
         for (int w = tid; w < NBL * T; w += NT) {
             const int t = w % T, bf = w / T;
             double2 a[RL];
@@ -218,33 +190,6 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_fwd_tuned(c
 #pragma unroll
             for (int j = 0; j < RL; j++) X[F::sw(bf + NBL * j, t)] = a[j];
         }
-    } else {
-        // outputs to the XOR-swizzled tile X[row][t ^ ((row / R0) % T)] (conflict-free for this pass and the next)
-        for (int w = tid; w < NB0 * T; w += NT) {
-            const int bf = w % NB0, t = w / NB0;
-            double2 a[R0];
-#pragma unroll
-            for (int k = 0; k < R0; k++) a[k] = t < nc ? Wb[(size_t)t * L + bf + k * NB0] : make_double2(0.0, 0.0);
-            Dft<R0, -1>::run(a);
-            tw_mul<R0, -1>(a, tw, bf);
-            const int tx = t ^ (bf % T);
-#pragma unroll
-            for (int j = 0; j < R0; j++) X[(bf * R0 + j) * T + tx] = a[j];
-        }
-        __syncthreads();
-        mid_pass<LT, R1, -1, T, NT>(
-            R0, tw, [&](int row, int t) { return X[row * T + (t ^ ((row / R0) % T))]; },
-            [&](int row, int t, double2 v) { Y[row * TP + t] = v; });
-        __syncthreads();
-        for (int w = tid; w < NBL * T; w += NT) {
-            const int t = w % T, bf = w / T;
-            double2 a[RL];
-#pragma unroll
-            for (int k = 0; k < RL; k++) a[k] = Y[(bf + k * NBL) * TP + t];
-            Dft<RL, -1>::run(a);
-#pragma unroll
-            for (int j = 0; j < RL; j++) X[(bf + NBL * j) * TP + t] = a[j];
-        }
     }
     __syncthreads();
     // gather the sphere runs (contiguous in n) and add the kinetic term
@@ -253,11 +198,10 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_fwd_tuned(c
     double2 *Ob = outC + (size_t)b * nG;
     for (int e = tid; e < nend - nbeg; e += NT) {
         const int n = nbeg + e;
-        int t = 0;
-        while (n >= s_n0[t + 1]) t++;
+        const int t = find_col<T>(s_n0, n);
         int row = s_m2w[t] + (n - s_n0[t]);
         if (row >= L) row -= L;
-        double2 v = F::NP == 2 ? X[F::sw(row, t)] : X[row * TP + t];
+        double2 v = X[F::sw(row, t)];
         v.x *= scale;
         v.y *= scale;
         if (kin != 0.0) {

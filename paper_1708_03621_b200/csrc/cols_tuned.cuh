@@ -25,7 +25,7 @@ struct Cfg {
     static constexpr int T = NP == 3 ? 8 : 16;                  // pencils per CTA
     static constexpr int TP = T + 1;
     // resident CTAs per SM the register allocation is bounded for (latency-bound kernels: more warps in flight win)
-    static constexpr int MINB = (LT == 128 || LT == 216) ? 4 : 6;
+    static constexpr int MINB_INV = LT == 128 ? 4 : (LT == 216 ? 5 : 6), MINB_FWD = (LT == 128 || LT == 216) ? 4 : 6;
     static constexpr int NBL = ok ? LT / RL : 1;                // butterflies per pencil in the last pass
     static constexpr int NB0 = ok ? LT / R0 : 1;                // ... in the first pass
     // ONE swizzled tile [L][T]; the shared -> shared passes run in a single round (threads = their work items) and
@@ -84,7 +84,7 @@ __device__ __forceinline__ void mid_pass_inplace(double2 *X, const double2 *__re
 
 // ------------------------------------------------------------------------------------------------ K1
 template <int LT>
-__global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_inv_tuned(const double2 *__restrict__ tw, const int ncol,
+__global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tuned(const double2 *__restrict__ tw, const int ncol,
                                                                 const int64_t nG, const int *__restrict__ col_n0,
                                                                 const int *__restrict__ col_m2lo,
                                                                 const double2 *__restrict__ C, double2 *__restrict__ W1) {
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_inv_tuned(c
 // ------------------------------------------------------------------------------------------------ K5
 // out[b][n] = scale * (F_2 W1)[column of n][m2 of n]  (+ kin * ke[n] * C[b][n])
 template <int LT>
-__global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB) k_cols_fwd_tuned(const double2 *__restrict__ tw, const int ncol,
+__global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_FWD) k_cols_fwd_tuned(const double2 *__restrict__ tw, const int ncol,
                                                                 const int64_t nG, const int *__restrict__ col_n0,
                                                                 const int *__restrict__ col_m2lo,
                                                                 const double2 *__restrict__ W1, const double scale,

@@ -236,7 +236,7 @@ __device__ __forceinline__ void twiddle_rows(double2 (&a)[R], const double2 *__r
 // resident CTAs per SM the register allocation of k_planes_fused is bounded for (measured: profiles/r01_planes_tuning.md)
 template <int LT> struct PlanesMinB { static constexpr int v = 4; };
 #ifndef PLANES_MINB_80
-#define PLANES_MINB_80 5
+#define PLANES_MINB_80 6
 #endif
 template <> struct PlanesMinB<80> { static constexpr int v = PLANES_MINB_80; };
 template <> struct PlanesMinB<72> { static constexpr int v = 6; };

@@ -76,13 +76,16 @@ int jdft_basis_export(const jdft_basis *b, int32_t *iG_host, int32_t *index_host
 int jdft_basis_device_maps(const jdft_basis *b, const int32_t **index_dev, const double **ke_dev);
 
 /* ---- workspace -------------------------------------------------------------------------------------
- * Bytes needed to process `nbands_batch` bands at once (FFT intermediates) and to run the projector /
- * overlap GEMMs with up to `nrows_max` rows (max of nproj, nb) -- the two phases share the buffer.
+ * Bytes needed to process `nbands_batch` bands at once (FFT intermediates) plus the projector / overlap GEMM
+ * scratch for up to `nrows_max` rows (max of nproj, nb).
  * Calls with more bands than fit are split into band batches internally (results are identical).      */
 size_t jdft_workspace_bytes(const jdft_basis *b, int nbands_batch, int nrows_max);
 int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
-/* tunables: "band_batch" (bands per FFT batch, 0 = automatic), "force_generic_fft" (0/1: use the
- * runtime-radix FFT kernels even for lengths that have specialised ones; for tests), "profile_kernel"  */
+/* tunables: "band_batch" (bands per FFT batch, 0 = automatic: what the workspace holds, at most 64),
+ * "force_generic_fft" (0/1: use the runtime-radix FFT kernels even for lengths that have specialised ones; for
+ * tests), "overlap_gemm" (0/1, default 0: apply_H forks B = D P^+ C onto a basis-owned side stream beside the FFT
+ * pipeline and joins before HC += P B; uses basis-owned events, so not for concurrent calls on one basis),
+ * "profile_kernel" (see diagnostics)                                                                    */
 int jdft_set_option(jdft_basis *b, const char *key, int64_t value);
 
 /* ---- operators ------------------------------------------------------ */

@@ -79,9 +79,36 @@ extern "C" int jdft_apply_H(const jdft_basis *b, const double *Vloc, const doubl
     if (!Vloc) return jdft_fail(JDFT_EINVAL, "apply_H: null Vloc");
     if (nb == 0) return JDFT_OK;
     cudaStream_t st = (cudaStream_t)s;
-    if ((rc = jdft_local_H(b, Vloc, C, nb, HC, st))) return rc;
-    if (nproj > 0) return vnl_impl(b, P, nproj, D, D_mode, C, nb, HC, 1, st, "apply_H");
-    return JDFT_OK;
+    if (nproj == 0) return jdft_local_H(b, Vloc, C, nb, HC, st);
+    // Fork/join: B = D P^+ C (DMMA pipe) runs on the basis' side stream while the FFT pipeline (shared-memory / FP64
+    // pipes) runs on the caller's stream; HC += P B follows both.  Needs separate workspace regions for the two.
+    const size_t bsz = align_up((size_t)nb * nproj * 16);
+    size_t part_bytes = b->ws_bytes / 4 < ((size_t)64 << 20) ? b->ws_bytes / 4 : ((size_t)64 << 20);
+    part_bytes &= ~(size_t)255;
+    const size_t gemm_bytes = 2 * bsz + part_bytes;
+    const bool fork = b->opt_overlap && b->side && b->ws && part_bytes >= (size_t)nb * nproj * 16 &&
+                      jdft_band_batch(b, nb, gemm_bytes) > 0;
+    if (!fork) {
+        if ((rc = jdft_local_H(b, Vloc, C, nb, HC, st))) return rc;
+        return vnl_impl(b, P, nproj, D, D_mode, C, nb, HC, 1, st, "apply_H");
+    }
+    char *ws = (char *)b->ws;
+    double *B1 = (double *)ws, *B2 = (double *)(ws + bsz);
+    void *part = ws + 2 * bsz;
+    JDFT_CUDA(cudaEventRecord(b->ev_fork, st));
+    JDFT_CUDA(cudaStreamWaitEvent(b->side, b->ev_fork, 0));
+    int rc_side = jdft_gemm_dotk(b, C, nb, P, nproj, b->nG, 1, 1.0, D_mode == 0 ? D : nullptr, B1, part, part_bytes, b->side);
+    const double *Bd = B1;
+    if (!rc_side && D_mode == 1) {
+        rc_side = jdft_gemm_dotk(b, B1, nb, D, nproj, nproj, 0, 1.0, nullptr, B2, part, part_bytes, b->side);
+        Bd = B2;
+    }
+    cudaEventRecord(b->ev_join, b->side);
+    rc = jdft_local_H(b, Vloc, C, nb, HC, st, gemm_bytes);
+    JDFT_CUDA(cudaStreamWaitEvent(st, b->ev_join, 0));  // always join, also on error
+    if (rc_side) return rc_side;
+    if (rc) return rc;
+    return jdft_gemm_expand(b, Bd, nb, P, nproj, b->nG, HC, 1, st);
 }
 
 extern "C" int jdft_overlap(const jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M,

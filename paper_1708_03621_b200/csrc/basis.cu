@@ -88,6 +88,9 @@ extern "C" int jdft_basis_destroy(jdft_basis *b) {
     cudaFree(b->d_rowcol);
     cudaFree(b->d_planeof);
     for (int d = 0; d < 3; d++) cudaFree(b->d_tw[d]);
+    if (b->side) cudaStreamDestroy(b->side);
+    if (b->ev_fork) cudaEventDestroy(b->ev_fork);
+    if (b->ev_join) cudaEventDestroy(b->ev_join);
     for (int i = 0; i < 8; i++) cudaFree(b->hb[i]);
     for (cudaEvent_t e : b->prof_ev) cudaEventDestroy(e);
     delete b;
@@ -120,6 +123,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     for (int i = 0; i < 8; i++) { b->hb[i] = nullptr; b->hb_bytes[i] = 0; }
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
     b->opt_profile_kernel = 0; b->prof_used = 0;
+    b->opt_overlap = 0; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
 
     // G = 2 pi R^-1 (adjugate / det): row i of G is the reciprocal vector b_i
     {
@@ -256,6 +260,9 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     if (e == cudaSuccess) e = upload(&b->d_rowcol, rowcol.data(), rowcol.size());
     if (e == cudaSuccess) e = upload(&b->d_planeof, planeof.data(), planeof.size());
     for (int d = 0; d < 3 && e == cudaSuccess; d++) e = upload(&b->d_tw[d], tw[d].data(), tw[d].size());
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&b->side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&b->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&b->ev_join, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         jdft_basis_destroy(b);
         return jdft_cuda_fail(e, "basis_create upload");
@@ -311,7 +318,7 @@ extern "C" size_t jdft_workspace_bytes(const jdft_basis *b, int nbands_batch, in
     if (!b) return 0;
     const size_t f = jdft_fft_bytes_per_band(b) * (size_t)(nbands_batch > 0 ? nbands_batch : 1);
     const size_t g = gemm_bytes(nrows_max);
-    return (f > g ? f : g) + 256;
+    return f + g + 512;  // both at once: the projection GEMM overlaps the FFT pipeline in apply_H
 }
 
 extern "C" int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes) {
@@ -325,15 +332,16 @@ extern "C" int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes) {
 extern "C" int jdft_set_option(jdft_basis *b, const char *key, int64_t value) {
     if (!b || !key) return jdft_fail(JDFT_EINVAL, "set_option: null argument");
     if (!strcmp(key, "band_batch")) { b->opt_band_batch = value < 0 ? 0 : value; return JDFT_OK; }
+    if (!strcmp(key, "overlap_gemm")) { b->opt_overlap = value != 0; return JDFT_OK; }
     if (!strcmp(key, "force_generic_fft")) { b->opt_force_generic = value != 0; return JDFT_OK; }
     if (!strcmp(key, "profile_kernel")) { b->opt_profile_kernel = value; b->prof_used = 0; return JDFT_OK; }
     return jdft_fail(JDFT_EINVAL, "set_option: unknown key '%s'", key);
 }
 
-int jdft_band_batch(const jdft_basis *b, int nb) {
+int jdft_band_batch(const jdft_basis *b, int nb, size_t ws_offset) {
     const size_t per = jdft_fft_bytes_per_band(b);
-    if (!b->ws || b->ws_bytes < per) return 0;
-    size_t fit = b->ws_bytes / per;
+    if (!b->ws || b->ws_bytes < ws_offset + per) return 0;
+    size_t fit = (b->ws_bytes - ws_offset) / per;
     int64_t want = b->opt_band_batch;
     if (want <= 0) {
         // automatic: as many bands as the workspace holds, up to 64.  Measured on B200 (profiles/r01_batch_sweep.md):

@@ -41,6 +41,11 @@ struct jdft_basis {
     size_t ws_bytes;
     // options
     int64_t opt_band_batch, opt_force_generic;
+    // fork/join resources of apply_H (option "overlap_gemm"): the projection GEMM runs on `side` while the FFT pipeline
+    // runs on the caller's stream
+    int64_t opt_overlap;
+    cudaStream_t side;
+    cudaEvent_t ev_fork, ev_join;
     // optional per-kernel event timing (option "profile_kernel" = one of JDFT_K_*; 0 = off).  Diagnostics only.
     int64_t opt_profile_kernel;
     std::vector<cudaEvent_t> prof_ev;  // pairs (begin, end)
@@ -75,10 +80,11 @@ void jdft_count_launch(int n);
 // per-band scratch of the FFT path (bytes)
 size_t jdft_fft_bytes_per_band(const jdft_basis *b);
 // bands per batch given the workspace and options; 0 if not even one fits
-int jdft_band_batch(const jdft_basis *b, int nb);
+int jdft_band_batch(const jdft_basis *b, int nb, size_t ws_offset = 0);
 
 // local.cu: FFT-based pieces
-int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C, int nb, double *HC, cudaStream_t st);
+int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C, int nb, double *HC, cudaStream_t st,
+                 size_t ws_offset = 0);  // the FFT intermediates start ws_offset bytes into the workspace
 
 // gemm.cu
 // Out[r][c] = scale * dscale[c] * sum_k X[r][k] * (conjY ? conj(Y[c][k]) : Y[c][k]);  X [Rn][K], Y [Cn][K], Out [Rn][Cn]

@@ -404,9 +404,9 @@ struct Bufs {
     double2 *W1, *W2;
 };
 
-Bufs carve(const jdft_basis *b, int nbatch) {
+Bufs carve(const jdft_basis *b, int nbatch, size_t ws_offset = 0) {
     Bufs w;
-    w.W1 = reinterpret_cast<double2 *>(b->ws);
+    w.W1 = reinterpret_cast<double2 *>(static_cast<char *>(b->ws) + ws_offset);
     w.W2 = w.W1 + (size_t)nbatch * b->ncol * b->S[2];
     return w;
 }
@@ -513,15 +513,16 @@ int check_common(const jdft_basis *b, const void *in, const void *out, int nb, c
 }  // namespace
 
 // HC = I^+ (Vloc .* I C) + Omega ke C  for all nb bands, in band batches
-int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C_, int nb, double *HC_, cudaStream_t st) {
-    const int nbatch = jdft_band_batch(b, nb);
+int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C_, int nb, double *HC_, cudaStream_t st,
+                 size_t ws_offset) {
+    const int nbatch = jdft_band_batch(b, nb, ws_offset);
     if (nb > 0 && nbatch == 0) return jdft_fail(JDFT_EWORKSPACE, "apply_H: workspace missing or smaller than one band (%zu bytes)", jdft_fft_bytes_per_band(b));
     const double2 *C = reinterpret_cast<const double2 *>(C_);
     double2 *HC = reinterpret_cast<double2 *>(HC_);
     int rc;
     for (int b0 = 0; b0 < nb; b0 += nbatch) {
         const int nbt = nb - b0 < nbatch ? nb - b0 : nbatch;
-        const Bufs w = carve(b, nbatch);
+        const Bufs w = carve(b, nbatch, ws_offset);
         const double2 *Cb = C + (size_t)b0 * b->nG;
         if ((rc = launch_cols_inv(b, Cb, nbt, w.W1, st))) return rc;
         if ((rc = launch_rows<false>(b, nbt, w.W1, w.W2, st))) return rc;

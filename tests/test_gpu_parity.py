@@ -244,3 +244,22 @@ def test_launch_counter(case, jd):
     jd.jdft_launch_count(reset=True)
     jd.jdft_apply_H(case.gb, dev(case.V.reshape(-1)), dev(case.P), dev(case.D), dev(case.C))
     assert jd.jdft_launch_count() >= 8
+
+
+def test_overlap_gemm_option_matches(ref, jd):
+    """apply_H with the projection GEMM forked onto the side stream gives the same result (and matches the oracle)."""
+    for D_dense in (False, True):
+        c = Case(ref, jd, 102)
+        D = c.D
+        if D_dense:
+            rng = np.random.default_rng(23)
+            n = c.P.shape[0]
+            A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+            D = (A + A.conj().T) / 2
+        want = c.rb.apply_H(c.V, c.P, D, c.C)
+        args = (dev(c.V.reshape(-1)), dev(c.P), dev(D), dev(c.C))
+        a = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+        jd.jdft_set_option(c.gb, "overlap_gemm", 1)
+        b = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+        assert rel_err_per_band(a, want) <= TOL and rel_err_per_band(b, want) <= TOL
+        assert rel_err_per_band(a, b) <= 1e-13

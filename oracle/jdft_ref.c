@@ -495,3 +495,47 @@ int jdft_ref_overlap_entry(const jdft_ref_basis *b, const double *C1_, const dou
     out2[1] = b->volume * (double)si;
     return REF_OK;
 }
+
+/* ---- the steps right after / before H C in every SCF or minimiser iteration
+ * ("ElecVars": wavefunctions -> density -> potential; PAPER.md:76 integrals as dot products).
+ *
+ * subspace:  M[a + nb1*bb] = sum_n conj(C1[a][n]) X2[bb][n]      (no Omega: X2 = H C already carries it)
+ * density:   n[j] (+)= sum_b f[b] |(I C_b)[j]|^2                 (I as defined above; f = occupations, real)  */
+int jdft_ref_subspace(const jdft_ref_basis *b, const double *C1_, int nb1, const double *X2_, int nb2, double *M_) {
+    if (!b || !C1_ || !X2_ || !M_ || nb1 < 0 || nb2 < 0) return REF_EINVAL;
+    const cplx *C1 = (const cplx *)C1_, *X2 = (const cplx *)X2_;
+    cplx *M = (cplx *)M_;
+    const int64_t nG = b->nG;
+#pragma omp parallel for schedule(dynamic) collapse(2)
+    for (int bb = 0; bb < nb2; bb++)
+        for (int a = 0; a < nb1; a++) {
+            long double sr = 0.0L, si = 0.0L;
+            for (int64_t n = 0; n < nG; n++) {
+                long double ar = creal(C1[(size_t)a * nG + n]), ai = cimag(C1[(size_t)a * nG + n]);
+                long double cr = creal(X2[(size_t)bb * nG + n]), ci = cimag(X2[(size_t)bb * nG + n]);
+                sr += ar * cr + ai * ci;
+                si += ar * ci - ai * cr;
+            }
+            M[(size_t)a + (size_t)nb1 * bb] = (double)sr + I * (double)si;
+        }
+    return REF_OK;
+}
+
+int jdft_ref_density(const jdft_ref_basis *b, const double *C_, int nb, const double *f, double *n, int accumulate) {
+    if (!b || !n || nb < 0 || (nb > 0 && (!C_ || !f))) return REF_EINVAL;
+    const cplx *C = (const cplx *)C_;
+    if (!accumulate) memset(n, 0, sizeof(double) * b->N);
+    cplx *box = (cplx *)malloc(sizeof(cplx) * b->N);
+    if (!box) return REF_ENOMEM;
+    for (int ib = 0; ib < nb; ib++) { /* bands one after the other, in order: a fixed summation order */
+        memset(box, 0, sizeof(cplx) * b->N);
+        for (int64_t g = 0; g < b->nG; g++) box[b->index[g]] = C[(size_t)ib * b->nG + g];
+        if (fft3d(box, b->S, +1)) { free(box); return REF_ENOMEM; }
+        for (int64_t j = 0; j < b->N; j++) {
+            const double re = creal(box[j]), im = cimag(box[j]);
+            n[j] += f[ib] * (re * re + im * im);
+        }
+    }
+    free(box);
+    return REF_OK;
+}

@@ -54,6 +54,8 @@ def lib():
         L.jdft_ref_apply_H.argtypes = [vp, vp, vp, ci, vp, ci, vp, ci, vp]
         L.jdft_ref_overlap.argtypes = [vp, vp, ci, vp, ci, vp]
         L.jdft_ref_overlap_entry.argtypes = [vp, vp, vp, ci, ci, vp]
+        L.jdft_ref_subspace.argtypes = [vp, vp, ci, vp, ci, vp]
+        L.jdft_ref_density.argtypes = [vp, vp, ci, vp, vp, ci]
         _lib = L
     return _lib
 
@@ -192,6 +194,25 @@ class RefBasis:
         M = np.empty((nb2, nb1), dtype=np.complex128)  # column-major nb1 x nb2 == C-order [nb2][nb1]
         _chk(lib().jdft_ref_overlap(self._h, _p(C1), nb1, _p(C2), nb2, _p(M)))
         return M.T  # M[a, b]
+
+    def subspace(self, C1, X2):
+        """M[a, b] = sum_n conj(C1[a, n]) X2[b, n] (no Omega); used as C^+ (H C)."""
+        C1, X2 = _c128(C1), _c128(X2)
+        nb1, nb2 = C1.shape[0], X2.shape[0]
+        M = np.empty((nb2, nb1), dtype=np.complex128)
+        _chk(lib().jdft_ref_subspace(self._h, _p(C1), nb1, _p(X2), nb2, _p(M)))
+        return M.T
+
+    def density(self, C, f, n=None):
+        """n[j] (+)= sum_b f[b] |(I C_b)[j]|^2, float64 [S0, S1, S2]; accumulates into n if given."""
+        C = _c128(C)
+        f = np.ascontiguousarray(f, dtype=np.float64)
+        acc = n is not None
+        if n is None:
+            n = np.zeros(self.shape, dtype=np.float64)
+        assert n.flags.c_contiguous and n.dtype == np.float64
+        _chk(lib().jdft_ref_density(self._h, _p(C), C.shape[0], _p(f), _p(n), 1 if acc else 0))
+        return n
 
     def overlap_entry(self, C1, C2, a, b):
         C1, C2 = _c128(C1), _c128(C2)

@@ -334,3 +334,77 @@ def test_translation_covariance(ref):
     # projectors carry exp(-2 pi i (m + k).x): the k part is a global phase per atom and cancels in P D P^+
     HC2 = b.apply_H(V2, P2, D, C * ph[None, :])
     assert np.max(np.abs(HC2 - ph[None, :] * HC)) <= 1e-12 * np.max(np.abs(HC))
+
+
+# ------------------------------------------------------------------------------------------ SURVEY 8(f) rank 1
+# subspace matrix C1^+ X2 and density n = sum_b f_b |I C_b|^2 (PAPER.md:127 ElecVars: wavefunctions -> density)
+
+def test_density_vs_explicit_matrix_closed_forms_and_invariants(ref):
+    rng = np.random.default_rng(41)
+    b = ref.RefBasis(_skew_lattice(), [0.2, -0.1, 0.3], 6.0, (8, 9, 10))
+    nb = 4
+    C = _rand_c(rng, nb, b.nG)
+    f = np.array([2.0, 1.5, 0.25, 0.0])
+    n = b.density(C, f)
+    # brute force: explicit N x nG matrix of I (independent of the oracle's FFT)
+    psi = (_brute_I_matrix(b) @ C.T).T.reshape((nb,) + b.shape)
+    want = np.einsum("b,bijk->ijk", f, np.abs(psi) ** 2)
+    assert np.max(np.abs(n - want)) <= 1e-11 * np.max(want)
+    # Parseval: sum_j n[j] = N sum_b f_b sum_n |C_b[n]|^2 ; with quadrature weight Omega/N this is sum_b f_b C_b^+ O C_b
+    assert abs(n.sum() - b.N * np.sum(f * np.sum(np.abs(C) ** 2, axis=1))) <= 1e-11 * n.sum()
+    assert abs(n.sum() * b.volume / b.N - np.sum(f * np.real(np.diag(b.overlap(C, C))))) <= 1e-10 * n.sum()
+    # real, non-negative, linear in f, accumulate adds, a band with f = 0 contributes nothing
+    assert n.min() >= 0.0
+    assert np.max(np.abs(b.density(C, 3.0 * f) - 3.0 * n)) <= 1e-12 * n.max()
+    assert np.max(np.abs(b.density(C[:3], f[:3]) - n)) == 0.0
+    acc = b.density(C[:2], f[:2])
+    b.density(C[2:], f[2:], acc)
+    assert np.max(np.abs(acc - n)) <= 1e-13 * n.max()
+    # one plane wave: constant density f |c|^2 ; two plane waves: closed-form cosine with the + sign convention of I
+    n1, n2 = 5, b.nG - 7
+    e = np.zeros((1, b.nG), dtype=np.complex128)
+    e[0, n1] = 0.3 - 0.4j
+    assert np.max(np.abs(b.density(e, [2.0]) - 2.0 * 0.25)) <= 1e-14
+    c1, c2 = 0.7 + 0.2j, -0.3 + 0.5j
+    e[0, n1], e[0, n2] = c1, c2
+    S = np.asarray(b.shape, dtype=np.float64)
+    j = np.stack(np.meshgrid(*[np.arange(s) for s in b.shape], indexing="ij"), -1)
+    dm = (b.iG[n1] - b.iG[n2]).astype(np.float64)
+    phase = 2 * np.pi * (j * dm / S).sum(-1)
+    want2 = abs(c1) ** 2 + abs(c2) ** 2 + 2 * np.real(c1 * np.conj(c2) * np.exp(1j * phase))
+    assert np.max(np.abs(b.density(e, [1.0]) - want2)) <= 1e-13
+
+
+def test_density_translation_covariance(ref):
+    """C'_m = exp(-2 pi i m.s/S) C_m shifts psi, hence the density, by the grid vector s."""
+    rng = np.random.default_rng(43)
+    b = ref.RefBasis(np.diag([6.0, 7.0, 8.0]), [0.0, 0.0, 0.0], 5.0, (10, 12, 9))
+    C = _rand_c(rng, 2, b.nG)
+    f = np.array([1.0, 0.5])
+    s = np.array([3, 5, 2])
+    ph = np.exp(-2j * np.pi * (b.iG * s / np.asarray(b.shape, dtype=np.float64)).sum(-1))
+    n0 = b.density(C, f)
+    n1 = b.density(C * ph[None, :], f)
+    assert np.max(np.abs(n1 - np.roll(n0, tuple(s), axis=(0, 1, 2)))) <= 1e-12 * n0.max()
+
+
+def test_subspace_vs_numpy_and_hermitian_for_H(ref):
+    rng = np.random.default_rng(47)
+    cfg = 101
+    R, kpts, Ecut, S = workloads.lattice(cfg)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    inp = workloads.make_inputs(cfg, b.iG)
+    C, X = inp["C"], _rand_c(rng, 3, b.nG)
+    M = b.subspace(C, X)
+    assert M.shape == (C.shape[0], 3)
+    assert np.max(np.abs(M - C.conj() @ X.T)) <= 1e-13 * np.max(np.abs(M))           # library matmul
+    assert np.max(np.abs(b.subspace(C, C) * b.volume - b.overlap(C, C))) <= 1e-13    # overlap = Omega * subspace
+    HC = b.apply_H(inp["Vloc"], inp["P"], inp["D"], C)
+    Hs = b.subspace(C, HC)
+    assert np.max(np.abs(Hs - Hs.conj().T)) <= 1e-12 * np.max(np.abs(Hs))            # Hermitian H => Hermitian C^+ H C
+    # Rayleigh quotient of a plane wave under constant V0: (ke[n] + V0) Omega
+    e = np.zeros((1, b.nG), dtype=np.complex128)
+    e[0, 11] = 1.0
+    V0 = 0.37
+    Vc = np.full(b.shape, V0 * b.volume / b.N)
+    assert abs(b.subspace(e, b.apply_H(Vc, None, None, e))[0, 0] - (b.ke[11] + V0) * b.volume) <= 1e-12 * b.volume

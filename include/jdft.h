@@ -113,6 +113,17 @@ int jdft_apply_H(const jdft_basis *b, const double *Vloc, const double *P, int n
 int jdft_overlap(const jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M,
                  jdft_stream s);
 
+/* ---- the steps next to H C in an SCF / minimiser iteration (PAPER.md:127 ElecVars:
+ * wavefunctions -> density -> potential; PAPER.md:76 integrals as dot products) ------------------------------ */
+/* subspace matrix: M[a + nb1*bb] = sum_n conj(C1[a][n]) X2[bb][n]  (column-major nb1 x nb2, c128; NO Omega --
+ * with X2 = H C1 this is the subspace Hamiltonian C^+ H C)                                                   */
+int jdft_subspace(const jdft_basis *b, const double *C1, int nb1, const double *X2, int nb2, double *M,
+                  jdft_stream s);
+/* density: n[j] (+)= sum_b f[b] |(I C_b)[j]|^2.  f = f64[nb] occupations (DEVICE), n = f64[N] (DEVICE), bands are
+ * summed in index order (deterministic); accumulate != 0 adds to the existing n.  psi never reaches HBM.      */
+int jdft_density(const jdft_basis *b, const double *C, int nb, const double *f, double *n, int accumulate,
+                 jdft_stream s);
+
 /* ---- HOST-buffer variants (end-to-end path: H2D copy, kernels, D2H copy, sync) -------------------- */
 int jdft_apply_H_host(jdft_basis *b, const double *Vloc_host, const double *P_host, int nproj,
                       const double *D_host, int D_mode, const double *C_host, int nb, double *HC_host);

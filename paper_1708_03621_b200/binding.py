@@ -19,7 +19,7 @@ EXPORTS = [
     "jdft_basis_create", "jdft_basis_destroy", "jdft_basis_info", "jdft_basis_structure", "jdft_basis_export",
     "jdft_basis_device_maps", "jdft_workspace_bytes", "jdft_set_workspace", "jdft_set_option",
     "jdft_apply_I", "jdft_apply_Idag", "jdft_apply_J", "jdft_apply_L", "jdft_apply_O", "jdft_apply_Vnl",
-    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_H_host", "jdft_overlap_host",
+    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_subspace", "jdft_density", "jdft_apply_H_host", "jdft_overlap_host",
     "jdft_last_error", "jdft_launch_count", "jdft_profile_read", "jdft_version",
 ]
 
@@ -52,6 +52,8 @@ def _load():
     L.jdft_project.argtypes = [vp, vp, ci, vp, ci, vp, vp]
     L.jdft_apply_H.argtypes = [vp, vp, vp, ci, vp, ci, vp, ci, vp, vp]
     L.jdft_overlap.argtypes = [vp, vp, ci, vp, ci, vp, vp]
+    L.jdft_subspace.argtypes = [vp, vp, ci, vp, ci, vp, vp]
+    L.jdft_density.argtypes = [vp, vp, ci, vp, vp, ci, vp]
     L.jdft_apply_H_host.argtypes = [vp, vp, vp, ci, vp, ci, vp, ci, vp]
     L.jdft_overlap_host.argtypes = [vp, vp, ci, vp, ci, vp]
     L.jdft_last_error.restype = ctypes.c_char_p
@@ -261,6 +263,31 @@ def jdft_overlap(basis, C1, C2, M=None):
     _chk(_lib.jdft_overlap(basis._h, _dev(C1, torch.complex128, "C1"), nb1, _dev(C2, torch.complex128, "C2"), nb2,
                            _dev(M, torch.complex128, "M"), _stream()))
     return M.t()
+
+
+def jdft_subspace(basis, C1, X2, M=None):
+    """Returns M with M[a, b] = sum_n conj(C1[a, n]) X2[b, n] (no Omega; a view of the column-major result)."""
+    nb1, nb2 = _bands(C1, basis, "C1"), _bands(X2, basis, "X2")
+    if M is None:
+        M = torch.empty((nb2, nb1), dtype=torch.complex128, device=C1.device)
+    _chk(_lib.jdft_subspace(basis._h, _dev(C1, torch.complex128, "C1"), nb1, _dev(X2, torch.complex128, "X2"), nb2,
+                            _dev(M, torch.complex128, "M"), _stream()))
+    return M.t()
+
+
+def jdft_density(basis, C, f, n=None, accumulate=False):
+    """n[S0, S1, S2] (+)= sum_b f[b] |(I C_b)|^2 ; f is a CUDA float64 tensor [nb]."""
+    nb = _bands(C, basis, "C")
+    if f.numel() != nb:
+        raise ValueError("f must have one entry per band")
+    if n is None:
+        n = torch.empty(basis.S, dtype=torch.float64, device=C.device)
+        accumulate = False
+    elif n.numel() != basis.N:
+        raise ValueError("n must have N = S0*S1*S2 entries")
+    _chk(_lib.jdft_density(basis._h, _dev(C, torch.complex128, "C"), nb, _dev(f, torch.float64, "f"),
+                           _dev(n, torch.float64, "n"), 1 if accumulate else 0, _stream()))
+    return n
 
 
 def _host(a, dtype, name):

@@ -124,6 +124,19 @@ extern "C" int jdft_overlap(const jdft_basis *b, const double *C1, int nb1, cons
     return jdft_gemm_dotk(b, C2, nb2, C1, nb1, b->nG, 1, b->volume, nullptr, M, b->ws, b->ws_bytes, (cudaStream_t)s);
 }
 
+extern "C" int jdft_subspace(const jdft_basis *b, const double *C1, int nb1, const double *X2, int nb2, double *M,
+                             jdft_stream s) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "subspace: null basis");
+    if (nb1 < 0 || nb2 < 0) return jdft_fail(JDFT_EINVAL, "subspace: negative size");
+    if (nb1 == 0 || nb2 == 0) return JDFT_OK;
+    if (!C1 || !X2 || !M) return jdft_fail(JDFT_EINVAL, "subspace: null data pointer");
+    int rc;
+    if ((rc = check_ptr16(C1, "subspace")) || (rc = check_ptr16(X2, "subspace")) || (rc = check_ptr16(M, "subspace"))) return rc;
+    if (!b->ws) return jdft_fail(JDFT_EWORKSPACE, "subspace: no workspace set");
+    // column-major nb1 x nb2 == row-major [nb2][nb1]:  M[bb][a] = sum_n X2[bb][n] conj(C1[a][n])
+    return jdft_gemm_dotk(b, X2, nb2, C1, nb1, b->nG, 1, 1.0, nullptr, M, b->ws, b->ws_bytes, (cudaStream_t)s);
+}
+
 // ---- HOST-buffer variants ----------------------------------------------------------------------------------
 namespace {
 int host_buf(jdft_basis *b, int slot, size_t bytes, void **out) {

@@ -368,6 +368,49 @@ __global__ void __launch_bounds__(Tuned<LT>::NT) k_rows_tuned(const double2 *__r
     }
 }
 
+// ------------------------------------------------------------------------------------------------ density
+// n[j] (+)= sum_b f[b] |psi_b[j]|^2 for the nbt bands of a batch: the last pass of I with an
+// accumulate-|psi|^2 epilogue instead of a store.  One CTA owns a tile (i1, kT adjacent i2) of the box and walks the
+// bands of the batch in order, so the sum has a fixed order and needs no atomics; psi never reaches HBM.
+template <int LT>
+__global__ void __launch_bounds__(kNT) k_planes_density(const FftPlan plan, const double2 *__restrict__ tw, const int S1,
+                                                        const int S2, const int npl, const int *__restrict__ planeof,
+                                                        const double2 *__restrict__ W2, const double *__restrict__ f,
+                                                        const int nbt, double *__restrict__ n, const int accumulate) {
+    constexpr int T = kT, TP = kT, NT = kNT;
+    const int L = LT > 0 ? LT : plan.L;  // = S0
+    extern __shared__ double2 smem[];
+    double2 *bufA = smem, *bufB = smem + L * TP;
+    double *acc = reinterpret_cast<double *>(smem + 2 * L * TP);
+    int *s_planeof = reinterpret_cast<int *>(acc + L * TP);
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y;
+    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    for (int i = tid; i < L * TP; i += NT) acc[i] = 0.0;
+    __syncthreads();
+    const size_t plane = (size_t)S1 * S2;
+    const int tmax = S2 - t0;
+    for (int b = 0; b < nbt; b++) {
+        const double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
+        const double fb = f[b];
+        fft_run<LT, +1, T, TP, NT>(
+            plan, tw, bufA, bufB,
+            [&](int row, int t) {
+                const int p = s_planeof[row];
+                return (p >= 0 && t < tmax) ? W2b[p * plane + t] : make_double2(0.0, 0.0);
+            },
+            [&](int row, int t, double2 v) { acc[row * TP + t] += fb * (v.x * v.x + v.y * v.y); });
+        __syncthreads();
+    }
+    double *nb_ = n + (size_t)i1 * S2 + t0;
+    for (int e = tid; e < L * T; e += NT) {
+        const int row = e / T, t = e - row * T;
+        if (t < tmax) {
+            double *o = nb_ + (size_t)row * plane + t;
+            *o = accumulate ? *o + acc[row * TP + t] : acc[row * TP + t];
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ diagonal ops
 // out[b][n] = (f0 + f1 * ke[n]) * C[b][n]
 __global__ void k_diag(const int64_t nG, const int64_t total, const double f0, const double f1,
@@ -577,6 +620,42 @@ extern "C" int jdft_apply_Idag(const jdft_basis *b, const double *psi, int nb, d
 extern "C" int jdft_apply_J(const jdft_basis *b, const double *psi, int nb, double *C, jdft_stream s) {
     if (!b) return jdft_fail(JDFT_EINVAL, "apply_J: null basis");
     return idag_scaled(b, psi, nb, C, 1.0 / (double)b->N, s, "apply_J");
+}
+
+extern "C" int jdft_density(const jdft_basis *b, const double *C_, int nb, const double *f, double *n, int accumulate,
+                            jdft_stream s) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "density: null basis");
+    if (nb < 0) return jdft_fail(JDFT_EINVAL, "density: negative band count");
+    if (!n || (nb > 0 && (!C_ || !f))) return jdft_fail(JDFT_EINVAL, "density: null data pointer");
+    if (((uintptr_t)C_) & 15) return jdft_fail(JDFT_EINVAL, "density: C not 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)s;
+    if (nb == 0) {
+        if (!accumulate) JDFT_CUDA(cudaMemsetAsync(n, 0, (size_t)b->N * 8, st));
+        return JDFT_OK;
+    }
+    const int nbatch = jdft_band_batch(b, nb);
+    if (nbatch == 0) return jdft_fail(JDFT_EWORKSPACE, "density: workspace missing or smaller than one band");
+    const double2 *C = reinterpret_cast<const double2 *>(C_);
+    const int L = b->S[0];
+    const size_t smem = 2 * (size_t)L * kT * sizeof(double2) + (size_t)L * kT * sizeof(double) + (size_t)L * sizeof(int);
+    dim3 grid((b->S[2] + kT - 1) / kT, b->S[1]);
+    int rc;
+    for (int b0 = 0; b0 < nb; b0 += nbatch) {
+        const int nbt = nb - b0 < nbatch ? nb - b0 : nbatch;
+        const Bufs w = carve(b, nbatch);
+        if ((rc = launch_cols_inv(b, C + (size_t)b0 * b->nG, nbt, w.W1, st))) return rc;
+        if ((rc = launch_rows<false>(b, nbt, w.W1, w.W2, st))) return rc;
+        const int acc = (accumulate || b0 > 0) ? 1 : 0;
+        jdft_prof_begin(b, JDFT_K_PLANES, st);
+        SPEC_SWITCH(L, b->opt_force_generic, {
+            JDFT_CUDA(ensure_smem(k_planes_density<LT>, smem));
+            k_planes_density<LT><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
+                                                          f + b0, nbt, n, acc);
+        });
+        jdft_prof_end(b, JDFT_K_PLANES, st);
+        JDFT_LAUNCH_CHECK("k_planes_density");
+    }
+    return JDFT_OK;
 }
 
 static int diag_op(const jdft_basis *b, const double *C, int nb, double *out, double f0, double f1, jdft_stream s,

@@ -108,3 +108,27 @@ def test_full_overlap_sampled_entries(full, jd):
         assert abs(M2[a, b] - want) <= TOL * colnorm[b], (a, b)
         want1 = full.rb.overlap_entry(full.C, full.C, a, b)
         assert abs(M[a, b] - want1) <= TOL
+
+
+def test_full_density_and_subspace(full, jd):
+    """Density of a band subset spanning several batches (the oracle sums bands serially) and the full subspace
+    Hamiltonian C^+ (H C) on sampled entries."""
+    nbd = 128 if full.cfg_id == 2 else 12
+    rng = np.random.default_rng(53)
+    f = rng.uniform(0.0, 2.0, nbd)
+    if full.cfg_id != 2:
+        jd.jdft_set_option(full.gb, "band_batch", 5)            # 5 + 5 + 2 bands
+    got = jd.jdft_density(full.gb, full.dC[:nbd].contiguous(), dev(f)).cpu().numpy()
+    jd.jdft_set_option(full.gb, "band_batch", 0)
+    want = full.rb.density(full.C[:nbd], f)
+    assert np.linalg.norm(got - want) <= TOL * np.linalg.norm(want)
+    # sum_j n[j] Omega/N = sum_b f_b (bands are O-orthonormal): holds at any size
+    assert abs(got.sum() * full.gb.volume / full.gb.N - f.sum()) <= 1e-11 * f.sum()
+    HC = jd.jdft_apply_H(full.gb, full.dV, full.dP, full.dD, full.dC)
+    Hs = jd.jdft_subspace(full.gb, full.dC, HC).cpu().numpy()
+    assert np.max(np.abs(Hs - Hs.conj().T)) <= 1e-12 * np.max(np.abs(Hs))
+    HCh = HC.cpu().numpy()
+    colnorm = np.linalg.norm(Hs, axis=0)
+    for a, b in [(0, 0), (full.nb - 1, 1), (3, full.nb - 1), (full.nb // 2, full.nb // 2 + 1)]:
+        want_ab = np.vdot(full.C[a], HCh[b])                    # one entry at a time, plain definition
+        assert abs(Hs[a, b] - want_ab) <= TOL * colnorm[b]

@@ -263,3 +263,41 @@ def test_overlap_gemm_option_matches(ref, jd):
         b = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
         assert rel_err_per_band(a, want) <= TOL and rel_err_per_band(b, want) <= TOL
         assert rel_err_per_band(a, b) <= 1e-13
+
+
+# ------------------------------------------------------------------------------------------ SURVEY 8(f) rank 1
+
+def test_subspace(case, jd):
+    rng = np.random.default_rng(31)
+    X = rng.standard_normal((3, case.rb.nG)) + 1j * rng.standard_normal((3, case.rb.nG))
+    want = case.rb.subspace(case.C, X)
+    got = jd.jdft_subspace(case.gb, dev(case.C), dev(X)).cpu().numpy()
+    assert got.shape == want.shape
+    assert rel_err_per_band(got.T, want.T) <= TOL
+    # C^+ (H C) from the GPU's own H C is Hermitian
+    HC = jd.jdft_apply_H(case.gb, dev(case.V.reshape(-1)), dev(case.P), dev(case.D), dev(case.C))
+    Hs = jd.jdft_subspace(case.gb, dev(case.C), HC).cpu().numpy()
+    assert np.max(np.abs(Hs - Hs.conj().T)) <= 1e-12 * np.max(np.abs(Hs))
+
+
+def test_density(case, jd):
+    rng = np.random.default_rng(37)
+    f = rng.uniform(0.0, 2.0, case.nb)
+    want = case.rb.density(case.C, f)
+    got = jd.jdft_density(case.gb, dev(case.C), dev(f)).cpu().numpy()
+    assert np.linalg.norm(got - want) <= TOL * np.linalg.norm(want)
+    assert got.min() >= 0.0
+    # accumulate into an existing array; batches of 1 and 3 bands give the same sum to rounding
+    base = rng.uniform(0.0, 1.0, case.rb.shape)
+    n = dev(base)
+    jd.jdft_density(case.gb, dev(case.C), dev(f), n, accumulate=True)
+    assert np.linalg.norm(n.cpu().numpy() - (base + want)) <= TOL * np.linalg.norm(base + want)
+    for batch in (1, 3):
+        jd.jdft_set_option(case.gb, "band_batch", batch)
+        g2 = jd.jdft_density(case.gb, dev(case.C), dev(f)).cpu().numpy()
+        assert np.linalg.norm(g2 - got) <= 1e-13 * np.linalg.norm(got)
+    jd.jdft_set_option(case.gb, "band_batch", 0)
+    # no bands: zeros
+    C0 = torch.empty((0, case.gb.nG), dtype=torch.complex128, device="cuda")
+    f0 = torch.empty((0,), dtype=torch.float64, device="cuda")
+    assert float(jd.jdft_density(case.gb, C0, f0).abs().max()) == 0.0

@@ -352,6 +352,33 @@ def run_ours(args):
               (2 * h["C"].numel() * 16 if do_overlap else 0) for h in host)
     d2h = sum(h["HC"].numel() * 16 + (h["M"].numel() * 16 if do_overlap else 0) for h in host)
 
+    # SURVEY 8(f) rank 1 operations on the same inputs (k-point 0): density of all bands, subspace Hamiltonian C^+ (H C)
+    extras = None
+    if args.extras:
+        k = ks[0]
+        fo = torch.rand(nb, dtype=torch.float64, device="cuda")
+        nr = torch.empty(tuple(S), dtype=torch.float64, device="cuda")
+        Hs = torch.empty((nb, nb), dtype=torch.complex128, device="cuda")
+
+        def t_op(fn, reps=5):
+            fn()
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+            for a, b in ev:
+                flush.zero_()
+                a.record()
+                fn()
+                b.record()
+            torch.cuda.synchronize()
+            return float(np.mean([a.elapsed_time(b) for a, b in ev]))
+
+        ms_d = t_op(lambda: jd.jdft_density(k["gb"], k["C"], fo, nr))
+        ms_s = t_op(lambda: jd.jdft_subspace(k["gb"], k["C"], k["HC"], Hs))
+        i = k["info"]
+        nbat = (nb + 63) // 64
+        dens_bytes = nb * 16 * (i["nG"] + 2 * i["a"] + 2 * i["b"]) + nbat * 2 * 8 * i["N"]
+        extras = {"density": {"ms": ms_d, "bands_per_s": nb / (ms_d * 1e-3), "alg_GB/s": dens_bytes / (ms_d * 1e-3) / 1e9},
+                  "subspace": {"ms": ms_s, "TFLOP/s": 8.0 * nb * nb * i["nG"] / (ms_s * 1e-3) / 1e12}}
+
     if rank != 0:
         return
     hbm_peak, hbm_src = measured_peaks()
@@ -405,6 +432,8 @@ def run_ours(args):
         "fp64_peaks": {"dmma_tflops": dmma_peak, "dfma_tflops": dfma_peak, "source": fp_src},
         "wall_s_timed_region": t_wall,
     }
+    if args.extras:
+        line["extras"] = extras
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args.config)
     print(json.dumps(line), flush=True)
@@ -419,6 +448,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=0, help="bands per FFT batch (0 = automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extras", action="store_true", help="also time jdft_density and jdft_subspace (SURVEY 8(f) rank 1)")
     ap.add_argument("--overlap", action="store_true",
                     help="run the projection GEMM on a side stream beside the FFT pipeline (measured +1-2 %; off by default)")
     args = ap.parse_args()

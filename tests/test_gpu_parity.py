@@ -301,3 +301,35 @@ def test_density(case, jd):
     C0 = torch.empty((0, case.gb.nG), dtype=torch.complex128, device="cuda")
     f0 = torch.empty((0,), dtype=torch.float64, device="cuda")
     assert float(jd.jdft_density(case.gb, C0, f0).abs().max()) == 0.0
+
+
+# ------------------------------------------------------------------------------------------ general lattices
+
+@pytest.mark.parametrize("S,k,Ecut", [((24, 20, 18), (0.2, -0.3, 0.1), 5.0), ((32, 27, 30), (0.0, 0.0, 0.0), 7.0),
+                                      ((16, 16, 50), (0.5, 0.5, 0.25), 4.0)])
+def test_skew_lattice_basis_and_H(ref, jd, S, k, Ecut):
+    """Non-orthogonal cell (the workload generator only makes orthorhombic ones): index maps bit-exact, H, I, J, density
+    against the oracle with random V, P, D."""
+    R = np.array([[7.0, 0.9, -0.6], [0.4, 8.0, 1.1], [-0.7, 0.3, 9.0]])
+    rb = ref.RefBasis(R, k, Ecut, S)
+    gb = jd.jdft_basis_create(R, k, Ecut, S)
+    iG, index, ke = jd.jdft_basis_export(gb)
+    assert np.array_equal(iG, rb.iG) and np.array_equal(index, rb.index)
+    assert np.max(np.abs(ke - rb.ke)) <= 1e-14 * np.max(rb.ke)
+    rng = np.random.default_rng(61)
+    nb, npj = 7, 5
+    C = rng.standard_normal((nb, rb.nG)) + 1j * rng.standard_normal((nb, rb.nG))
+    P = rng.standard_normal((npj, rb.nG)) + 1j * rng.standard_normal((npj, rb.nG))
+    D = rng.uniform(-1, 1, npj)
+    V = rng.standard_normal(S) * (rb.volume / rb.N)
+    jd.jdft_alloc_workspace(gb, 4, 8)
+    want = rb.apply_H(V, P, D, C)
+    got = jd.jdft_apply_H(gb, dev(V.reshape(-1)), dev(P), dev(D), dev(C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+    psi = jd.jdft_apply_I(gb, dev(C))
+    assert rel_err_per_band(psi.cpu().numpy(), rb.apply_I(C)) <= TOL
+    assert rel_err_per_band(jd.jdft_apply_J(gb, psi).cpu().numpy(), C) <= 1e-13
+    f = rng.uniform(0, 2, nb)
+    n_want = rb.density(C, f)
+    n_got = jd.jdft_density(gb, dev(C), dev(f)).cpu().numpy()
+    assert np.linalg.norm(n_got - n_want) <= TOL * np.linalg.norm(n_want)

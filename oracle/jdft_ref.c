@@ -539,3 +539,70 @@ int jdft_ref_density(const jdft_ref_basis *b, const double *C_, int nb, const do
     free(box);
     return REF_OK;
 }
+
+/* ---- the scalar-field operators of the paper's Listing 1 and eq. (1)
+ * (PAPER.md:63):  -4 pi rho = div( epsilon grad phi ),
+ *     hessian(phi~) = (-1/(4 pi)) * divergence( J( epsilon * I( gradient(phi~) ) ) ).
+ * "the gradient and divergence operators apply in reciprocal space (where they are diagonal)":
+ *     gradient:   out[d][n] = i q_d(n) phi[n],  q(n) = G^T (iG[n] + k)  (Cartesian, d = 0,1,2)
+ *     divergence: out[n]    = sum_d i q_d(n) X[d][n]
+ * Layouts: a field block is [nb][nG]; a vector-field block is [3][nb][nG] (component slowest).  epsilon is f64[N].
+ * Reading (#23): I, J exactly as above (J = I^+/N), no extra volume factors.               */
+static void qvec(const jdft_ref_basis *b, int64_t n, double *q) {
+    const double t[3] = {b->iG[3 * n] + b->k[0], b->iG[3 * n + 1] + b->k[1], b->iG[3 * n + 2] + b->k[2]};
+    for (int d = 0; d < 3; d++) q[d] = b->G[0 + d] * t[0] + b->G[3 + d] * t[1] + b->G[6 + d] * t[2]; /* (G^T t)_d */
+}
+
+int jdft_ref_gradient(const jdft_ref_basis *b, const double *C_, int nb, double *out_) {
+    if (!b || nb < 0 || (nb > 0 && (!C_ || !out_))) return REF_EINVAL;
+    const cplx *C = (const cplx *)C_;
+    cplx *out = (cplx *)out_;
+    const size_t blk = (size_t)nb * b->nG;
+    for (int ib = 0; ib < nb; ib++)
+        for (int64_t n = 0; n < b->nG; n++) {
+            double q[3];
+            qvec(b, n, q);
+            for (int d = 0; d < 3; d++) out[d * blk + (size_t)ib * b->nG + n] = (I * q[d]) * C[(size_t)ib * b->nG + n];
+        }
+    return REF_OK;
+}
+
+int jdft_ref_divergence(const jdft_ref_basis *b, const double *X_, int nb, double *out_) {
+    if (!b || nb < 0 || (nb > 0 && (!X_ || !out_))) return REF_EINVAL;
+    const cplx *X = (const cplx *)X_;
+    cplx *out = (cplx *)out_;
+    const size_t blk = (size_t)nb * b->nG;
+    for (int ib = 0; ib < nb; ib++)
+        for (int64_t n = 0; n < b->nG; n++) {
+            double q[3];
+            qvec(b, n, q);
+            cplx s = 0.0;
+            for (int d = 0; d < 3; d++) s += (I * q[d]) * X[d * blk + (size_t)ib * b->nG + n];
+            out[(size_t)ib * b->nG + n] = s;
+        }
+    return REF_OK;
+}
+
+int jdft_ref_pcm_hessian(const jdft_ref_basis *b, const double *epsilon, const double *phi, int nb, double *out) {
+    if (!b || nb < 0 || !epsilon || (nb > 0 && (!phi || !out))) return REF_EINVAL;
+    const size_t blk = (size_t)nb * b->nG;
+    double *g = (double *)malloc(sizeof(cplx) * 3 * blk);          /* gradient(phi) and later J(...)      */
+    double *r = (double *)malloc(sizeof(cplx) * 3 * (size_t)nb * b->N); /* I(gradient(phi))             */
+    if (!g || !r) { free(g); free(r); return REF_ENOMEM; }
+    int rc = jdft_ref_gradient(b, phi, nb, g);
+    if (!rc) rc = jdft_ref_apply_I(b, g, 3 * nb, r);
+    if (!rc) {
+        cplx *rr = (cplx *)r;
+        for (size_t f = 0; f < (size_t)3 * nb; f++)
+            for (int64_t j = 0; j < b->N; j++) rr[f * b->N + j] *= epsilon[j];      /* epsilon * (...)   */
+        rc = jdft_ref_apply_J(b, r, 3 * nb, g);
+    }
+    if (!rc) rc = jdft_ref_divergence(b, g, nb, out);
+    if (!rc) {
+        cplx *o = (cplx *)out;
+        for (size_t i = 0; i < blk; i++) o[i] *= -1.0 / (4.0 * M_PI);
+    }
+    free(g);
+    free(r);
+    return rc;
+}

@@ -56,6 +56,9 @@ def lib():
         L.jdft_ref_overlap_entry.argtypes = [vp, vp, vp, ci, ci, vp]
         L.jdft_ref_subspace.argtypes = [vp, vp, ci, vp, ci, vp]
         L.jdft_ref_density.argtypes = [vp, vp, ci, vp, vp, ci]
+        L.jdft_ref_gradient.argtypes = [vp, vp, ci, vp]
+        L.jdft_ref_divergence.argtypes = [vp, vp, ci, vp]
+        L.jdft_ref_pcm_hessian.argtypes = [vp, vp, vp, ci, vp]
         _lib = L
     return _lib
 
@@ -213,6 +216,29 @@ class RefBasis:
         assert n.flags.c_contiguous and n.dtype == np.float64
         _chk(lib().jdft_ref_density(self._h, _p(C), C.shape[0], _p(f), _p(n), 1 if acc else 0))
         return n
+
+    def gradient(self, C):
+        """[3, nb, nG]: i q_d C, q = G^T (iG + k) Cartesian."""
+        C = _c128(C)
+        out = np.empty((3,) + C.shape, dtype=np.complex128)
+        _chk(lib().jdft_ref_gradient(self._h, _p(C), C.shape[0], _p(out)))
+        return out
+
+    def divergence(self, X):
+        """[nb, nG]: sum_d i q_d X[d]."""
+        X = _c128(X)
+        out = np.empty(X.shape[1:], dtype=np.complex128)
+        _chk(lib().jdft_ref_divergence(self._h, _p(X), X.shape[1], _p(out)))
+        return out
+
+    def pcm_hessian(self, epsilon, phi):
+        """Listing 1 of the paper: (-1/4 pi) divergence(J(epsilon * I(gradient(phi)))); epsilon float64 [S0,S1,S2]."""
+        phi = _c128(phi)
+        eps = np.ascontiguousarray(epsilon, dtype=np.float64)
+        assert eps.size == self.N
+        out = np.empty_like(phi)
+        _chk(lib().jdft_ref_pcm_hessian(self._h, _p(eps), _p(phi), phi.shape[0], _p(out)))
+        return out
 
     def overlap_entry(self, C1, C2, a, b):
         C1, C2 = _c128(C1), _c128(C2)

@@ -408,3 +408,71 @@ def test_subspace_vs_numpy_and_hermitian_for_H(ref):
     V0 = 0.37
     Vc = np.full(b.shape, V0 * b.volume / b.N)
     assert abs(b.subspace(e, b.apply_H(Vc, None, None, e))[0, 0] - (b.ke[11] + V0) * b.volume) <= 1e-12 * b.volume
+
+
+# ------------------------------------------------------------------------------------------ SURVEY 8(f) rank 3
+# Listing 1 of the paper: hessian(phi) = (-1/4 pi) divergence(J(epsilon * I(gradient(phi))))
+
+def _q_cart(b, R, k):
+    """Cartesian q = 2 pi R^-T (m + k), computed here with numpy (not by the oracle)."""
+    return (b.iG.astype(np.float64) + np.asarray(k, dtype=np.float64)) @ (2 * np.pi * np.linalg.inv(R))
+
+
+def test_gradient_divergence_closed_forms_and_finite_differences(ref):
+    rng = np.random.default_rng(71)
+    R, k = _skew_lattice(), [0.0, 0.0, 0.0]
+    b = ref.RefBasis(R, k, 5.0, (10, 12, 9))
+    q = _q_cart(b, R, k)
+    phi = _rand_c(rng, 2, b.nG)
+    g = b.gradient(phi)
+    assert g.shape == (3, 2, b.nG)
+    for d in range(3):
+        assert np.max(np.abs(g[d] - 1j * q[None, :, d] * phi)) <= 1e-13 * np.max(np.abs(g))
+    # div grad = -|q|^2 = -2 ke = L / Omega
+    lap = b.divergence(g)
+    assert np.max(np.abs(lap - (-2.0 * b.ke)[None, :] * phi)) <= 1e-12 * np.max(np.abs(lap))
+    assert np.max(np.abs(lap * b.volume - b.apply_L(phi))) <= 1e-12 * np.max(np.abs(lap)) * b.volume
+    # real-space meaning: I(gradient(phi))_d is the Cartesian derivative of f(r) = sum_n phi_n exp(i q_n . r)
+    # (central differences of the explicitly evaluated sum at three grid points; r_j = R (j / S))
+    S = np.asarray(b.shape, dtype=np.float64)
+    Ig = b.apply_I(g.reshape(6, b.nG)).reshape((3, 2) + b.shape)
+
+    def f(r):
+        return (phi[0] * np.exp(1j * (q @ r))).sum()
+
+    h = 1e-5
+    for j in [(0, 0, 0), (3, 7, 2), (9, 11, 8)]:
+        r = R @ (np.asarray(j) / S)
+        for d in range(3):
+            e = np.zeros(3)
+            e[d] = h
+            fd = (f(r + e) - f(r - e)) / (2 * h)
+            assert abs(Ig[d, 0][j] - fd) <= 1e-6 * max(1.0, abs(fd))
+
+
+def test_pcm_hessian_vs_explicit_matrices_constant_epsilon_and_hermiticity(ref):
+    rng = np.random.default_rng(73)
+    R, k = _skew_lattice(), [0.0, 0.0, 0.0]
+    b = ref.RefBasis(R, k, 4.0, (8, 9, 8))
+    q = _q_cart(b, R, k)
+    eps = 1.0 + 78.0 * rng.random(b.shape)                   # an inhomogeneous dielectric between 1 and 79
+    phi = _rand_c(rng, 3, b.nG)
+    got = b.pcm_hessian(eps, phi)
+    # brute force from the explicit N x nG matrix of I: (-1/4pi) sum_d Dg_d (1/N) I^H diag(eps) I Dg_d
+    Im = _brute_I_matrix(b)
+    K = (Im.conj().T * eps.reshape(-1)[None, :]) @ Im / b.N
+    want = np.zeros_like(phi)
+    for d in range(3):
+        Dg = 1j * q[:, d]
+        want += (Dg[None, :] * ((K @ (Dg[None, :] * phi).T).T))
+    want *= -1.0 / (4 * np.pi)
+    assert np.max(np.abs(got - want)) <= 1e-11 * np.max(np.abs(want))
+    # constant epsilon: J I = 1  =>  hessian = (eps0 / 4 pi) |q|^2 phi   (eq. (1) of the paper with constant epsilon)
+    e0 = 78.4
+    got0 = b.pcm_hessian(np.full(b.shape, e0), phi)
+    assert np.max(np.abs(got0 - (e0 / (4 * np.pi)) * (2.0 * b.ke)[None, :] * phi)) <= 1e-12 * np.max(np.abs(got0))
+    # Hermitian (and positive) for real positive epsilon
+    a_, b_ = phi[0], phi[1]
+    Ha, Hb = got[0], got[1]
+    assert abs(np.vdot(a_, Hb) - np.conj(np.vdot(b_, Ha))) <= 1e-12 * np.linalg.norm(a_) * np.linalg.norm(Hb)
+    assert np.real(np.vdot(a_, Ha)) > 0

@@ -124,6 +124,18 @@ int jdft_subspace(const jdft_basis *b, const double *C1, int nb1, const double *
 int jdft_density(const jdft_basis *b, const double *C, int nb, const double *f, double *n, int accumulate,
                  jdft_stream s);
 
+/* ---- scalar-field operators of the paper's Listing 1 --------
+ * gradient:   out[d][b][n] = i q_d(n) C[b][n],  q = G^T (iG[n] + k) Cartesian, d = 0,1,2;  out is [3][nb][nG]
+ * divergence: out[b][n]    = sum_d i q_d(n) X[d][b][n];                                     X   is [3][nb][nG]
+ * pcm_hessian (Listing 1): out = (-1/(4 pi)) divergence(J(epsilon .* I(gradient(phi)))), epsilon f64[N] real,
+ *   phi/out [nb][nG]; one fused pass: the epsilon multiply rides inside the FFT pipeline, nothing of size N per
+ *   field reaches HBM.  Needs workspace for 3 nb nG c128 plus FFT scratch (jdft_workspace_bytes(b, 3 nb, 0) +
+ *   48 nb nG is enough).                                                                                     */
+int jdft_gradient(const jdft_basis *b, const double *C, int nb, double *out, jdft_stream s);
+int jdft_divergence(const jdft_basis *b, const double *X, int nb, double *out, jdft_stream s);
+int jdft_pcm_hessian(const jdft_basis *b, const double *epsilon, const double *phi, int nb, double *out,
+                     jdft_stream s);
+
 /* ---- HOST-buffer variants (end-to-end path: H2D copy, kernels, D2H copy, sync) -------------------- */
 int jdft_apply_H_host(jdft_basis *b, const double *Vloc_host, const double *P_host, int nproj,
                       const double *D_host, int D_mode, const double *C_host, int nb, double *HC_host);

@@ -19,7 +19,7 @@ EXPORTS = [
     "jdft_basis_create", "jdft_basis_destroy", "jdft_basis_info", "jdft_basis_structure", "jdft_basis_export",
     "jdft_basis_device_maps", "jdft_workspace_bytes", "jdft_set_workspace", "jdft_set_option",
     "jdft_apply_I", "jdft_apply_Idag", "jdft_apply_J", "jdft_apply_L", "jdft_apply_O", "jdft_apply_Vnl",
-    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_subspace", "jdft_density", "jdft_apply_H_host", "jdft_overlap_host",
+    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_apply_H_host", "jdft_overlap_host",
     "jdft_last_error", "jdft_launch_count", "jdft_profile_read", "jdft_version",
 ]
 
@@ -54,6 +54,9 @@ def _load():
     L.jdft_overlap.argtypes = [vp, vp, ci, vp, ci, vp, vp]
     L.jdft_subspace.argtypes = [vp, vp, ci, vp, ci, vp, vp]
     L.jdft_density.argtypes = [vp, vp, ci, vp, vp, ci, vp]
+    L.jdft_gradient.argtypes = [vp, vp, ci, vp, vp]
+    L.jdft_divergence.argtypes = [vp, vp, ci, vp, vp]
+    L.jdft_pcm_hessian.argtypes = [vp, vp, vp, ci, vp, vp]
     L.jdft_apply_H_host.argtypes = [vp, vp, vp, ci, vp, ci, vp, ci, vp]
     L.jdft_overlap_host.argtypes = [vp, vp, ci, vp, ci, vp]
     L.jdft_last_error.restype = ctypes.c_char_p
@@ -288,6 +291,38 @@ def jdft_density(basis, C, f, n=None, accumulate=False):
     _chk(_lib.jdft_density(basis._h, _dev(C, torch.complex128, "C"), nb, _dev(f, torch.float64, "f"),
                            _dev(n, torch.float64, "n"), 1 if accumulate else 0, _stream()))
     return n
+
+
+def jdft_gradient(basis, C, out=None):
+    """[3, nb, nG] = i q_d C."""
+    nb = _bands(C, basis, "C")
+    if out is None:
+        out = torch.empty((3, nb, basis.nG), dtype=torch.complex128, device=C.device)
+    _chk(_lib.jdft_gradient(basis._h, _dev(C, torch.complex128, "C"), nb, _dev(out, torch.complex128, "out"), _stream()))
+    return out
+
+
+def jdft_divergence(basis, X, out=None):
+    """[nb, nG] = sum_d i q_d X[d];  X is [3, nb, nG]."""
+    if X.dim() != 3 or X.shape[0] != 3 or X.shape[2] != basis.nG:
+        raise ValueError("X must have shape [3, nb, nG]")
+    nb = int(X.shape[1])
+    if out is None:
+        out = torch.empty((nb, basis.nG), dtype=torch.complex128, device=X.device)
+    _chk(_lib.jdft_divergence(basis._h, _dev(X, torch.complex128, "X"), nb, _dev(out, torch.complex128, "out"), _stream()))
+    return out
+
+
+def jdft_pcm_hessian(basis, epsilon, phi, out=None):
+    """Listing 1 of the paper: (-1/4 pi) divergence(J(epsilon * I(gradient(phi)))); epsilon float64 with N entries."""
+    nb = _bands(phi, basis, "phi")
+    if epsilon.numel() != basis.N:
+        raise ValueError("epsilon must have N = S0*S1*S2 entries")
+    if out is None:
+        out = torch.empty_like(phi)
+    _chk(_lib.jdft_pcm_hessian(basis._h, _dev(epsilon, torch.float64, "epsilon"), _dev(phi, torch.complex128, "phi"), nb,
+                               _dev(out, torch.complex128, "out"), _stream()))
+    return out
 
 
 def _host(a, dtype, name):

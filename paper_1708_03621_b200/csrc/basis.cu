@@ -82,6 +82,7 @@ extern "C" int jdft_basis_destroy(jdft_basis *b) {
     if (!b) return jdft_fail(JDFT_EINVAL, "basis_destroy: null basis");
     cudaSetDevice(b->device);
     cudaFree(b->d_index);
+    cudaFree(b->d_iG);
     cudaFree(b->d_ke);
     cudaFree(b->d_col_n0);
     cudaFree(b->d_col_m2lo);
@@ -117,7 +118,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     b->device = device;
     b->volume = std::fabs(det);
     b->N = (int64_t)S[0] * S[1] * S[2];
-    b->d_index = nullptr; b->d_ke = nullptr; b->d_col_n0 = nullptr; b->d_col_m2lo = nullptr;
+    b->d_index = nullptr; b->d_iG = nullptr; b->d_ke = nullptr; b->d_col_n0 = nullptr; b->d_col_m2lo = nullptr;
     b->d_rowcol = nullptr; b->d_planeof = nullptr;
     for (int d = 0; d < 3; d++) b->d_tw[d] = nullptr;
     for (int i = 0; i < 8; i++) { b->hb[i] = nullptr; b->hb_bytes[i] = 0; }
@@ -254,6 +255,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     // upload
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = upload(&b->d_index, b->index.data(), b->index.size());
+    if (e == cudaSuccess) e = upload(&b->d_iG, b->iG.data(), b->iG.size());
     if (e == cudaSuccess) e = upload(&b->d_ke, b->ke.data(), b->ke.size());
     if (e == cudaSuccess) e = upload(&b->d_col_n0, b->col_n0.data(), b->col_n0.size());
     if (e == cudaSuccess) e = upload(&b->d_col_m2lo, b->col_m2lo.data(), b->col_m2lo.size());

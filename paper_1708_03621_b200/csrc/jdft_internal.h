@@ -30,6 +30,7 @@ struct jdft_basis {
     std::vector<int> col_n0, col_m2lo;        // [ncol+1], [ncol]
     // device copies
     int32_t *d_index;
+    int32_t *d_iG;                            // [nG][3] (gradient / divergence)
     double *d_ke;
     int *d_col_n0, *d_col_m2lo;               // [ncol+1], [ncol]
     int *d_rowcol;                            // [npl][S1]: column index of (plane p, i1) or -1
@@ -83,8 +84,10 @@ size_t jdft_fft_bytes_per_band(const jdft_basis *b);
 int jdft_band_batch(const jdft_basis *b, int nb, size_t ws_offset = 0);
 
 // local.cu: FFT-based pieces
+// out = scale * I^+ (Vloc .* I C) + kin * ke .* C; the FFT intermediates start ws_offset bytes into the workspace.
+// kin < 0 selects the default Omega (the -1/2 L C term of H).  out may alias C when kin == 0.
 int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C, int nb, double *HC, cudaStream_t st,
-                 size_t ws_offset = 0);  // the FFT intermediates start ws_offset bytes into the workspace
+                 size_t ws_offset = 0, double scale = 1.0, double kin = -1.0);
 
 // gemm.cu
 // Out[r][c] = scale * dscale[c] * sum_k X[r][k] * (conjY ? conj(Y[c][k]) : Y[c][k]);  X [Rn][K], Y [Cn][K], Out [Rn][Cn]

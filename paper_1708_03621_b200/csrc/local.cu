@@ -6,6 +6,7 @@
 //   K4 k_rows<fwd>  forward FFT along axis 1, dense planes -> compact columns
 //   K5 k_cols_fwd   forward FFT along axis 2 (+) gather box -> sphere (+) + Omega ke C   (the -1/2 L C term)
 // Intermediates: W1 [nbatch][ncol][S2] and W2 [nbatch][npl][S1][S2] (c128) in the caller's workspace.
+#include <cmath>
 #include "fft.cuh"
 #include "cols_tuned.cuh"
 
@@ -411,6 +412,43 @@ __global__ void __launch_bounds__(kNT) k_planes_density(const FftPlan plan, cons
     }
 }
 
+// ------------------------------------------------------------------------------------------------ gradient / divergence
+// ("gradient and divergence operators apply in reciprocal space (where they are diagonal)")
+// q(n) = G^T (iG[n] + k) Cartesian; Gm = the 3x3 G row-major (row i = reciprocal vector b_i).
+struct Mat3 { double g[9], k[3]; };
+__device__ __forceinline__ void q_of(const Mat3 &m, const int32_t *__restrict__ iG, const int64_t n, double (&q)[3]) {
+    const double t0 = iG[3 * n] + m.k[0], t1 = iG[3 * n + 1] + m.k[1], t2 = iG[3 * n + 2] + m.k[2];
+#pragma unroll
+    for (int d = 0; d < 3; d++) q[d] = m.g[d] * t0 + m.g[3 + d] * t1 + m.g[6 + d] * t2;
+}
+// out[d][b][n] = i q_d C[b][n]
+__global__ void k_gradient(const Mat3 m, const int32_t *__restrict__ iG, const int64_t nG, const int64_t total,
+                           const double2 *__restrict__ C, double2 *__restrict__ out) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        double q[3];
+        q_of(m, iG, i % nG, q);
+        const double2 c = C[i];
+#pragma unroll
+        for (int d = 0; d < 3; d++) out[d * total + i] = make_double2(-q[d] * c.y, q[d] * c.x);
+    }
+}
+// out[b][n] = f * sum_d i q_d X[d][b][n]
+__global__ void k_divergence(const Mat3 m, const int32_t *__restrict__ iG, const int64_t nG, const int64_t total,
+                             const double f, const double2 *__restrict__ X, double2 *__restrict__ out) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        double q[3];
+        q_of(m, iG, i % nG, q);
+        double sr = 0.0, si = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            const double2 x = X[d * total + i];
+            sr -= q[d] * x.y;
+            si += q[d] * x.x;
+        }
+        out[i] = make_double2(f * sr, f * si);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ diagonal ops
 // out[b][n] = (f0 + f1 * ke[n]) * C[b][n]
 __global__ void k_diag(const int64_t nG, const int64_t total, const double f0, const double f1,
@@ -557,7 +595,8 @@ int check_common(const jdft_basis *b, const void *in, const void *out, int nb, c
 
 // HC = I^+ (Vloc .* I C) + Omega ke C  for all nb bands, in band batches
 int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C_, int nb, double *HC_, cudaStream_t st,
-                 size_t ws_offset) {
+                 size_t ws_offset, double scale, double kin) {
+    if (kin < 0.0) kin = b->volume;
     const int nbatch = jdft_band_batch(b, nb, ws_offset);
     if (nb > 0 && nbatch == 0) return jdft_fail(JDFT_EWORKSPACE, "apply_H: workspace missing or smaller than one band (%zu bytes)", jdft_fft_bytes_per_band(b));
     const double2 *C = reinterpret_cast<const double2 *>(C_);
@@ -571,7 +610,7 @@ int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C_, int 
         if ((rc = launch_rows<false>(b, nbt, w.W1, w.W2, st))) return rc;
         if ((rc = launch_planes<0>(b, nbt, w.W2, Vloc, nullptr, st))) return rc;
         if ((rc = launch_rows<true>(b, nbt, w.W1, w.W2, st))) return rc;
-        if ((rc = launch_cols_fwd(b, w.W1, nbt, 1.0, b->volume, Cb, HC + (size_t)b0 * b->nG, st))) return rc;
+        if ((rc = launch_cols_fwd(b, w.W1, nbt, scale, kin, Cb, HC + (size_t)b0 * b->nG, st))) return rc;
     }
     return JDFT_OK;
 }
@@ -656,6 +695,70 @@ extern "C" int jdft_density(const jdft_basis *b, const double *C_, int nb, const
         JDFT_LAUNCH_CHECK("k_planes_density");
     }
     return JDFT_OK;
+}
+
+namespace {
+Mat3 mat3_of(const jdft_basis *b) {
+    Mat3 m;
+    for (int i = 0; i < 9; i++) m.g[i] = b->G[i];
+    for (int i = 0; i < 3; i++) m.k[i] = b->k[i];
+    return m;
+}
+int elementwise_grid(int64_t total) {
+    int64_t blocks = (total + 255) / 256;
+    return (int)(blocks > 148 * 16 ? 148 * 16 : blocks);
+}
+int launch_gradient(const jdft_basis *b, const double *C, int nb, double *out, cudaStream_t st) {
+    const int64_t total = (int64_t)nb * b->nG;
+    jdft_prof_begin(b, JDFT_K_DIAG, st);
+    k_gradient<<<elementwise_grid(total), 256, 0, st>>>(mat3_of(b), b->d_iG, b->nG, total, reinterpret_cast<const double2 *>(C),
+                                                        reinterpret_cast<double2 *>(out));
+    jdft_prof_end(b, JDFT_K_DIAG, st);
+    JDFT_LAUNCH_CHECK("k_gradient");
+    return JDFT_OK;
+}
+int launch_divergence(const jdft_basis *b, const double *X, int nb, double f, double *out, cudaStream_t st) {
+    const int64_t total = (int64_t)nb * b->nG;
+    jdft_prof_begin(b, JDFT_K_DIAG, st);
+    k_divergence<<<elementwise_grid(total), 256, 0, st>>>(mat3_of(b), b->d_iG, b->nG, total, f, reinterpret_cast<const double2 *>(X),
+                                                          reinterpret_cast<double2 *>(out));
+    jdft_prof_end(b, JDFT_K_DIAG, st);
+    JDFT_LAUNCH_CHECK("k_divergence");
+    return JDFT_OK;
+}
+}  // namespace
+
+extern "C" int jdft_gradient(const jdft_basis *b, const double *C, int nb, double *out, jdft_stream s) {
+    int rc = check_common(b, C, out, nb, "gradient");
+    if (rc) return rc;
+    if (nb == 0) return JDFT_OK;
+    return launch_gradient(b, C, nb, out, (cudaStream_t)s);
+}
+
+extern "C" int jdft_divergence(const jdft_basis *b, const double *X, int nb, double *out, jdft_stream s) {
+    int rc = check_common(b, X, out, nb, "divergence");
+    if (rc) return rc;
+    if (nb == 0) return JDFT_OK;
+    return launch_divergence(b, X, nb, 1.0, out, (cudaStream_t)s);
+}
+
+// Listing 1 of the paper: hessian(phi) = (-1/4 pi) divergence(J(epsilon * I(gradient(phi)))).  The three gradient
+// components run through the fused pruned pipeline as 3 nb "bands" (epsilon multiply inside K3, 1/N of J in K5's
+// gather); the component block lives at the front of the workspace and is transformed in place.
+extern "C" int jdft_pcm_hessian(const jdft_basis *b, const double *epsilon, const double *phi, int nb, double *out,
+                                jdft_stream s) {
+    int rc = check_common(b, phi, out, nb, "pcm_hessian");
+    if (rc) return rc;
+    if (!epsilon) return jdft_fail(JDFT_EINVAL, "pcm_hessian: null epsilon");
+    if (nb == 0) return JDFT_OK;
+    cudaStream_t st = (cudaStream_t)s;
+    const size_t gbytes = (((size_t)3 * nb * b->nG * 16) + 255) & ~(size_t)255;
+    if (!b->ws || jdft_band_batch(b, 3 * nb, gbytes) == 0)
+        return jdft_fail(JDFT_EWORKSPACE, "pcm_hessian: workspace must hold 3 nb nG c128 (%zu bytes) plus one band of FFT scratch", gbytes);
+    double *g = static_cast<double *>(b->ws);
+    if ((rc = launch_gradient(b, phi, nb, g, st))) return rc;
+    if ((rc = jdft_local_H(b, epsilon, g, 3 * nb, g, st, gbytes, 1.0 / (double)b->N, 0.0))) return rc;
+    return launch_divergence(b, g, nb, -1.0 / (4.0 * M_PI), out, st);
 }
 
 static int diag_op(const jdft_basis *b, const double *C, int nb, double *out, double f0, double f1, jdft_stream s,

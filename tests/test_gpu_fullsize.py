@@ -132,3 +132,28 @@ def test_full_density_and_subspace(full, jd):
     for a, b in [(0, 0), (full.nb - 1, 1), (3, full.nb - 1), (full.nb // 2, full.nb // 2 + 1)]:
         want_ab = np.vdot(full.C[a], HCh[b])                    # one entry at a time, plain definition
         assert abs(Hs[a, b] - want_ab) <= TOL * colnorm[b]
+
+
+def test_full_pcm_hessian_scalar_field_basis(ref, jd):
+    """Listing 1 on a scalar-field basis of the density cutoff (4 x the wavefunction cutoff: sphere radius doubles and
+    just fits the box), config-2 box 80^3, Gamma: 8 fields at once, sampled fields against the oracle; constant epsilon
+    reduces to (eps0 / 4 pi) |q|^2 phi at any size."""
+    R, _, Ecut, S = workloads.lattice(2)
+    k = [0.0, 0.0, 0.0]
+    rb = ref.RefBasis(R, k, 4 * Ecut, S)
+    gb = jd.jdft_basis_create(R, k, 4 * Ecut, S)
+    iG, index, ke = jd.jdft_basis_export(gb)
+    assert np.array_equal(iG, rb.iG) and np.array_equal(index, rb.index)
+    rng = np.random.default_rng(97)
+    nf = 8
+    phi = rng.standard_normal((nf, rb.nG)) + 1j * rng.standard_normal((nf, rb.nG))
+    eps = 1.0 + 78.0 * rng.random(S)
+    ws = jd.jdft_workspace_bytes(gb, 3 * nf, 0) + 48 * nf * gb.nG
+    jd.jdft_set_workspace(gb, torch.empty(ws, dtype=torch.uint8, device="cuda"))
+    got = jd.jdft_pcm_hessian(gb, dev(eps.reshape(-1)), dev(phi)).cpu().numpy()
+    sample = [0, nf - 1]
+    want = rb.pcm_hessian(eps, phi[sample])
+    assert rel(got[sample], want) <= TOL
+    e0 = 78.4
+    got0 = jd.jdft_pcm_hessian(gb, dev(np.full(S, e0).reshape(-1)), dev(phi)).cpu().numpy()
+    assert rel(got0, (e0 / (4 * np.pi)) * (2.0 * ke)[None, :] * phi) <= 1e-12

@@ -333,3 +333,39 @@ def test_skew_lattice_basis_and_H(ref, jd, S, k, Ecut):
     n_want = rb.density(C, f)
     n_got = jd.jdft_density(gb, dev(C), dev(f)).cpu().numpy()
     assert np.linalg.norm(n_got - n_want) <= TOL * np.linalg.norm(n_want)
+
+
+# ------------------------------------------------------------------------------------------ SURVEY 8(f) rank 3 (Listing 1)
+
+def test_gradient_divergence(case, jd):
+    want = case.rb.gradient(case.C)
+    got = jd.jdft_gradient(case.gb, dev(case.C)).cpu().numpy()
+    assert got.shape == want.shape
+    for d in range(3):
+        assert rel_err_per_band(got[d], want[d]) <= 1e-14
+    rng = np.random.default_rng(83)
+    X = rng.standard_normal(want.shape) + 1j * rng.standard_normal(want.shape)
+    assert rel_err_per_band(jd.jdft_divergence(case.gb, dev(X)).cpu().numpy(), case.rb.divergence(X)) <= 1e-14
+
+
+def test_pcm_hessian(case, jd):
+    rng = np.random.default_rng(89)
+    eps = 1.0 + 78.0 * rng.random(case.rb.shape)
+    nb = min(case.nb, 5)
+    phi = np.ascontiguousarray(case.C[:nb])
+    want = case.rb.pcm_hessian(eps, phi)
+    ws = jd.jdft_workspace_bytes(case.gb, 3 * nb, 0) + 48 * nb * case.gb.nG
+    jd.jdft_set_workspace(case.gb, torch.empty(ws, dtype=torch.uint8, device="cuda"))
+    got = jd.jdft_pcm_hessian(case.gb, dev(eps.reshape(-1)), dev(phi)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+    # several band batches inside the call give the same result
+    jd.jdft_set_option(case.gb, "band_batch", 2)
+    got2 = jd.jdft_pcm_hessian(case.gb, dev(eps.reshape(-1)), dev(phi)).cpu().numpy()
+    jd.jdft_set_option(case.gb, "band_batch", 0)
+    assert rel_err_per_band(got2, got) <= 1e-13
+    # too small a workspace is refused
+    jd.jdft_set_workspace(case.gb, torch.empty(48 * nb * case.gb.nG, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(jd.JdftError) as e:
+        jd.jdft_pcm_hessian(case.gb, dev(eps.reshape(-1)), dev(phi))
+    assert e.value.code == jd.JDFT_EWORKSPACE
+    jd.jdft_alloc_workspace(case.gb, min(case.nb, 8), max(case.nb, case.P.shape[0]))

@@ -221,6 +221,13 @@ def algorithmic(cfgk, kernel, nbatches):
     return 0
 
 
+def overlap_flops(nb, nG):
+    """Real flops jdft_overlap(C, C) performs: C^+ C is Hermitian, so only the 64 x 64 tiles on and below the diagonal
+    are computed ("half if only the Hermitian triangle is computed -- then count half")."""
+    t = (nb + 63) // 64
+    return 8 * (t * (t + 1) // 2) * 64 * 64 * nG
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -258,7 +265,7 @@ def run_ours(args):
                        M=torch.empty((nb, nb), dtype=torch.complex128, device="cuda") if do_overlap else None,
                        C_h=C_h, P_h=P_h,
                        info=dict(nG=gb.nG, a=gb.ncol * S[2], b=gb.npl * S[1] * S[2], N=gb.N, nb=nb, nproj=nproj,
-                                 overlap_flops=8 * nb * nb * gb.nG if do_overlap else 0)))
+                                 overlap_flops=overlap_flops(nb, gb.nG) if do_overlap else 0)))
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
 
     def step():

@@ -106,7 +106,7 @@ class Basis:
 
     def __del__(self):
         h = getattr(self, "_h", None)
-        if h:
+        if h and _lib is not None:  # at interpreter shutdown the module globals may already be gone
             _lib.jdft_basis_destroy(h)
             self._h = None
 

@@ -52,12 +52,22 @@ __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld
 template <bool CONJY>
 __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
                                                         const double2 *__restrict__ Y, const int Cn, const int64_t K,
-                                                        const int ktiles_per_split, double2 *__restrict__ part) {
+                                                        const int ktiles_per_split, double2 *__restrict__ part,
+                                                        const int tri) {
     extern __shared__ __align__(16) char smem[];
     char *sX = smem, *sY = smem + STAGES * OPK_BYTES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wr = (warp >> 1) * 32, wc = (warp & 1) * 32;
-    const int row0 = blockIdx.y * BM, col0 = blockIdx.x * BN;
+    // tri: X == Y and the result is Hermitian; blockIdx.x enumerates the lower-triangle tiles (row tile >= col tile)
+    int tr = blockIdx.y, tc = blockIdx.x;
+    if (tri) {
+        const int t = blockIdx.x;
+        tr = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
+        while ((tr + 1) * (tr + 2) / 2 <= t) tr++;
+        while (tr * (tr + 1) / 2 > t) tr--;
+        tc = t - tr * (tr + 1) / 2;
+    }
+    const int row0 = tr * BM, col0 = tc * BN;
     const int64_t ktiles = (K + BK - 1) / BK;
     const int64_t kt0 = (int64_t)blockIdx.z * ktiles_per_split;
     int64_t kt1 = kt0 + ktiles_per_split;
@@ -129,15 +139,24 @@ __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restric
 }
 
 // Out[i] = scale * dscale[c] * sum_s part[s][i]   (fixed order)
+// tri: only tiles with row tile >= col tile were computed; the rest is the conjugate transpose (Hermitian result)
 __global__ void k_splitk_reduce(const double2 *__restrict__ part, const int nsplit, const int64_t total, const int Cn,
-                                const double scale, const double *__restrict__ dscale, double2 *__restrict__ Out) {
+                                const double scale, const double *__restrict__ dscale, double2 *__restrict__ Out,
+                                const int tri) {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        int64_t src = i;
+        bool cj = false;
+        if (tri) {
+            const int r = (int)(i / Cn), c = (int)(i % Cn);
+            if (c / BN > r / BM) { src = (int64_t)c * Cn + r; cj = true; }
+        }
         double sr = 0.0, si = 0.0;
         for (int s = 0; s < nsplit; s++) {
-            const double2 v = part[(size_t)s * total + i];
+            const double2 v = part[(size_t)s * total + src];
             sr += v.x;
             si += v.y;
         }
+        if (cj) si = -si;
         const double f = dscale ? scale * dscale[i % Cn] : scale;
         Out[i] = make_double2(f * sr, f * si);
     }
@@ -248,7 +267,10 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
                    cudaStream_t st) {
     if (Rn <= 0 || Cn <= 0) return JDFT_OK;
     const int64_t ktiles = (K + BK - 1) / BK;
-    const int tiles = ((Rn + BM - 1) / BM) * ((Cn + BN - 1) / BN);
+    // X^+ X is Hermitian: compute the lower-triangle tiles only and mirror them in the reduction
+    const int tri = (X == Y && Rn == Cn && conjY && !dscale && BM == BN) ? 1 : 0;
+    const int trow = (Rn + BM - 1) / BM;
+    const int tiles = tri ? trow * (trow + 1) / 2 : trow * ((Cn + BN - 1) / BN);
     const size_t one = (size_t)Rn * Cn * 16;
     // Split K so that the grid fills whole waves of the 148 SMs x 2 resident CTAs (184 registers x 128 threads):
     // among 1..6 waves take the first whose fill tiles*nsplit / (waves*slots) reaches 93 %, else the best one.
@@ -274,14 +296,14 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     nsplit = (ktiles + per - 1) / per;
     if (nsplit < 1) nsplit = 1;
     const size_t smem = 2 * STAGES * OPK_BYTES;
-    dim3 grid((Cn + BN - 1) / BN, (Rn + BM - 1) / BM, (unsigned)nsplit);
+    dim3 grid(tri ? tiles : (Cn + BN - 1) / BN, tri ? 1 : trow, (unsigned)nsplit);
     jdft_prof_begin(b, JDFT_K_GEMM_DOTK, st);
     if (conjY) {
         JDFT_CUDA(ensure_smem(k_gemm_dotk<true>, smem));
-        k_gemm_dotk<true><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
+        k_gemm_dotk<true><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch, tri);
     } else {
         JDFT_CUDA(ensure_smem(k_gemm_dotk<false>, smem));
-        k_gemm_dotk<false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
+        k_gemm_dotk<false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch, tri);
     }
     jdft_prof_end(b, JDFT_K_GEMM_DOTK, st);
     JDFT_LAUNCH_CHECK("k_gemm_dotk");
@@ -289,7 +311,7 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     int64_t blocks = (total + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
     jdft_prof_begin(b, JDFT_K_REDUCE, st);
-    k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, total, Cn, scale, dscale, (double2 *)Out);
+    k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, total, Cn, scale, dscale, (double2 *)Out, tri);
     jdft_prof_end(b, JDFT_K_REDUCE, st);
     JDFT_LAUNCH_CHECK("k_splitk_reduce");
     return JDFT_OK;

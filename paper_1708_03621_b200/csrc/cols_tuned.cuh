@@ -25,7 +25,11 @@ struct Cfg {
     static constexpr int T = NP == 3 ? 8 : 16;                  // pencils per CTA
     static constexpr int TP = T + 1;
     // resident CTAs per SM the register allocation is bounded for (latency-bound kernels: more warps in flight win)
-    static constexpr int MINB_INV = LT == 128 ? 4 : (LT == 216 ? 5 : 6), MINB_FWD = (LT == 128 || LT == 216) ? 4 : 6;
+    static constexpr int RMAX = R0 > R1 ? (R0 > R2 ? R0 : R2) : (R1 > R2 ? R1 : R2);
+    static constexpr int FIT = ok ? 65536 / (T * (LT / R0) * (RMAX >= 15 ? 80 : (RMAX >= 12 ? 72 : 40))) : 1;
+    static constexpr int MINB_DEF = FIT < 1 ? 1 : (FIT > 6 ? 6 : FIT);
+    // measured choices for the lengths of the five workloads (profiles/), the rule for the rest
+    static constexpr int MINB_INV = LT == 216 ? 5 : (LT == 128 ? 4 : MINB_DEF), MINB_FWD = (LT == 216 || LT == 128) ? 4 : MINB_DEF;
     static constexpr int NBL = ok ? LT / RL : 1;                // butterflies per pencil in the last pass
     static constexpr int NB0 = ok ? LT / R0 : 1;                // ... in the first pass
     // ONE swizzled tile [L][T]; the shared -> shared passes run in a single round (threads = their work items) and

@@ -8,7 +8,8 @@
 // ld(row, t) and the last pass hands its outputs to a store functor st(row, t, value), so callers fuse
 // the global-memory side (zero fill, pruning, V multiply, ...) into the butterflies.
 //
-// Lengths in SpecPlan<> run with compile-time radices up to 16 (two or three passes); any other
+// Lengths in SpecPlan<> (32 48 64 72 80 96 100 120 128 144 160 192 216 256) run with compile-time radices up to 16
+// (two or three passes); any other
 // 2/3/5-smooth length runs the same code with the radices 4, 2, 3, 5 taken from FftPlan at run time.
 #pragma once
 #include <cuda_runtime.h>
@@ -215,6 +216,14 @@ struct SpecPlan {
         static constexpr int radix(int i) { return i == 0 ? A : (i == 1 ? B : C); } \
     };
 JFFT_SPEC2(32, 4, 8)
+JFFT_SPEC2(48, 6, 8)
+JFFT_SPEC2(96, 8, 12)
+JFFT_SPEC2(100, 10, 10)
+JFFT_SPEC2(120, 8, 15)
+JFFT_SPEC2(144, 12, 12)
+JFFT_SPEC2(160, 10, 16)
+JFFT_SPEC2(192, 12, 16)
+JFFT_SPEC2(256, 16, 16)
 JFFT_SPEC2(64, 8, 8)
 JFFT_SPEC2(72, 8, 9)
 JFFT_SPEC2(80, 8, 10)
@@ -223,7 +232,13 @@ JFFT_SPEC3(216, 6, 6, 6)
 #undef JFFT_SPEC2
 #undef JFFT_SPEC3
 
-inline bool has_spec(int L) { return L == 32 || L == 64 || L == 72 || L == 80 || L == 128 || L == 216; }
+inline bool has_spec(int L) {
+    switch (L) {
+        case 32: case 48: case 64: case 72: case 80: case 96: case 100: case 120: case 128: case 144: case 160: case 192:
+        case 216: case 256: return true;
+        default: return false;
+    }
+}
 
 // ---------------------------------------------------------------- one Stockham pass
 // Current sub-length n = L / s (s = product of the radices already applied), m = n / R.

@@ -49,18 +49,17 @@ __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld
 }
 
 // ---------------------------------------------------------------------------------------------- dot-K GEMM
-template <bool CONJY>
+template <bool CONJY, bool TRI>
 __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
                                                         const double2 *__restrict__ Y, const int Cn, const int64_t K,
-                                                        const int ktiles_per_split, double2 *__restrict__ part,
-                                                        const int tri) {
+                                                        const int ktiles_per_split, double2 *__restrict__ part) {
     extern __shared__ __align__(16) char smem[];
     char *sX = smem, *sY = smem + STAGES * OPK_BYTES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wr = (warp >> 1) * 32, wc = (warp & 1) * 32;
     // tri: X == Y and the result is Hermitian; blockIdx.x enumerates the lower-triangle tiles (row tile >= col tile)
     int tr = blockIdx.y, tc = blockIdx.x;
-    if (tri) {
+    if constexpr (TRI) {
         const int t = blockIdx.x;
         tr = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
         while ((tr + 1) * (tr + 2) / 2 <= t) tr++;
@@ -298,12 +297,15 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     const size_t smem = 2 * STAGES * OPK_BYTES;
     dim3 grid(tri ? tiles : (Cn + BN - 1) / BN, tri ? 1 : trow, (unsigned)nsplit);
     jdft_prof_begin(b, JDFT_K_GEMM_DOTK, st);
-    if (conjY) {
-        JDFT_CUDA(ensure_smem(k_gemm_dotk<true>, smem));
-        k_gemm_dotk<true><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch, tri);
+    if (tri) {
+        JDFT_CUDA(ensure_smem(k_gemm_dotk<true, true>, smem));
+        k_gemm_dotk<true, true><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
+    } else if (conjY) {
+        JDFT_CUDA(ensure_smem(k_gemm_dotk<true, false>, smem));
+        k_gemm_dotk<true, false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
     } else {
-        JDFT_CUDA(ensure_smem(k_gemm_dotk<false>, smem));
-        k_gemm_dotk<false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch, tri);
+        JDFT_CUDA(ensure_smem(k_gemm_dotk<false, false>, smem));
+        k_gemm_dotk<false, false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
     }
     jdft_prof_end(b, JDFT_K_GEMM_DOTK, st);
     JDFT_LAUNCH_CHECK("k_gemm_dotk");

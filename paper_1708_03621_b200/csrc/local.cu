@@ -235,7 +235,12 @@ __device__ __forceinline__ void twiddle_rows(double2 (&a)[R], const double2 *__r
 }
 
 // resident CTAs per SM the register allocation of k_planes_fused is bounded for (measured: profiles/r01_planes_tuning.md)
-template <int LT> struct PlanesMinB { static constexpr int v = 4; };
+// default: registers the fused middle radix needs (16 complex values + V factors for radix 15/16) against 64 K per SM
+template <int LT> struct PlanesMinB {
+    static constexpr int need = Tuned<LT>::R2 >= 12 ? 128 : 96;
+    static constexpr int fit = 65536 / (Tuned<LT>::NT * need);
+    static constexpr int v = fit < 1 ? 1 : (fit > 6 ? 6 : fit);
+};
 #ifndef PLANES_MINB_80
 #define PLANES_MINB_80 6
 #endif
@@ -463,7 +468,7 @@ __global__ void k_diag(const int64_t nG, const int64_t total, const double f0, c
 // ------------------------------------------------------------------------------------------------ launch helpers
 template <class K>
 cudaError_t ensure_smem(K kernel, size_t bytes) {
-    if (bytes <= 48 * 1024) return cudaSuccess;
+    if (bytes <= 40 * 1024) return cudaSuccess;  // static __shared__ tables count against the 48 KB default too
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
@@ -472,6 +477,14 @@ cudaError_t ensure_smem(K kernel, size_t bytes) {
         const int l__ = (force_generic) ? 0 : (L);            \
         switch (l__) {                                        \
             case 32: { constexpr int LT = 32; __VA_ARGS__; } break;  \
+            case 48: { constexpr int LT = 48; __VA_ARGS__; } break;  \
+            case 96: { constexpr int LT = 96; __VA_ARGS__; } break;  \
+            case 100: { constexpr int LT = 100; __VA_ARGS__; } break; \
+            case 120: { constexpr int LT = 120; __VA_ARGS__; } break; \
+            case 144: { constexpr int LT = 144; __VA_ARGS__; } break; \
+            case 160: { constexpr int LT = 160; __VA_ARGS__; } break; \
+            case 192: { constexpr int LT = 192; __VA_ARGS__; } break; \
+            case 256: { constexpr int LT = 256; __VA_ARGS__; } break; \
             case 64: { constexpr int LT = 64; __VA_ARGS__; } break;  \
             case 72: { constexpr int LT = 72; __VA_ARGS__; } break;  \
             case 80: { constexpr int LT = 80; __VA_ARGS__; } break;  \

@@ -369,3 +369,23 @@ def test_pcm_hessian(case, jd):
         jd.jdft_pcm_hessian(case.gb, dev(eps.reshape(-1)), dev(phi))
     assert e.value.code == jd.JDFT_EWORKSPACE
     jd.jdft_alloc_workspace(case.gb, min(case.nb, 8), max(case.nb, case.P.shape[0]))
+
+
+# ------------------------------------------------------------------------------------------ every specialised length
+
+@pytest.mark.parametrize("cfg_id", list(range(201, 210)))
+def test_specialised_lengths_on_every_axis(ref, jd, cfg_id):
+    """48 96 100 120 144 160 192 256 each as the column, row and plane length: H, I, J and the density."""
+    c = Case(ref, jd, cfg_id)
+    iG, index, _ = jd.jdft_basis_export(c.gb)
+    assert np.array_equal(iG, c.rb.iG) and np.array_equal(index, c.rb.index)
+    want = c.rb.apply_H(c.V, c.P, c.D, c.C)
+    got = jd.jdft_apply_H(c.gb, dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+    psi = jd.jdft_apply_I(c.gb, dev(c.C))
+    assert rel_err_per_band(psi.cpu().numpy(), c.rb.apply_I(c.C)) <= TOL
+    assert rel_err_per_band(jd.jdft_apply_J(c.gb, psi).cpu().numpy(), c.C) <= 1e-13
+    f = np.array([1.0, 0.5, 2.0])
+    n_want = c.rb.density(c.C, f)
+    n_got = jd.jdft_density(c.gb, dev(c.C), dev(f)).cpu().numpy()
+    assert np.linalg.norm(n_got - n_want) <= TOL * np.linalg.norm(n_want)

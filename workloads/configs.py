@@ -35,6 +35,19 @@ TEST_CONFIGS = {
 }
 
 
+# Boxes that put every additional specialised FFT length (48 96 100 120 144 160 192 256) on every axis (each axis runs
+# different kernels: columns = axis 2, rows = axis 1, planes = axis 0); cell edge = S/4 bohr, Ecut 9 Ha => |m_d| <~ S_d/6.
+def _rot(name, S, cfg_id):
+    return dict(name=name, cell=tuple(s / 4.0 for s in S), kpoints=[(0.0, 0.0, 0.0) if cfg_id % 2 else (0.3, -0.2, 0.1)],
+                Ecut=9.0, S=S, nb=3, natoms=2, n_lm=4, atoms="uniform", extra="noise")
+
+
+_LEN_BOXES = [(48, 96, 100), (96, 100, 48), (100, 48, 96), (120, 144, 160), (144, 160, 120), (160, 120, 144),
+              (192, 256, 32), (256, 32, 192), (32, 192, 256)]
+for _i, _S in enumerate(_LEN_BOXES):
+    TEST_CONFIGS[201 + _i] = _rot("t_len_%dx%dx%d" % _S, _S, 201 + _i)
+
+
 def get_config(cfg_id):
     if cfg_id in CONFIGS:
         return CONFIGS[cfg_id]

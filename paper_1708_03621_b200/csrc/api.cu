@@ -176,19 +176,54 @@ extern "C" int jdft_apply_H_host(jdft_basis *b, const double *Vloc, const double
         b->ws = dW;
         b->ws_bytes = need;
     }
-    cudaStream_t st = 0;
-    cudaError_t e = cudaMemcpyAsync(dC, C, cb, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dV, Vloc, vb, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess && nproj > 0) e = cudaMemcpyAsync(dP, P, pb, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess && nproj > 0) e = cudaMemcpyAsync(dD, D, db, cudaMemcpyHostToDevice, st);
-    rc = e == cudaSuccess ? jdft_apply_H(b, (const double *)dV, (const double *)dP, nproj, (const double *)dD, D_mode,
-                                         (const double *)dC, nb, (double *)dHC, st)
-                          : jdft_cuda_fail(e, "apply_H_host H2D");
+    // Copy-in on the basis' side stream in the order the kernels need the data (C, Vloc, then P, D); the FFT pipeline
+    // starts as soon as C and Vloc have landed and runs while the (larger) projector block is still in flight; the
+    // projector GEMMs wait for the second event.  Pinned host buffers make the copies truly asynchronous.
+    cudaStream_t st = 0, cp = b->side ? b->side : (cudaStream_t)0;
+    cudaError_t e = cudaMemcpyAsync(dC, C, cb, cudaMemcpyHostToDevice, cp);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dV, Vloc, vb, cudaMemcpyHostToDevice, cp);
+    if (e == cudaSuccess && cp != st) e = cudaEventRecord(b->ev_fork, cp);
+    if (e == cudaSuccess && nproj > 0) e = cudaMemcpyAsync(dP, P, pb, cudaMemcpyHostToDevice, cp);
+    if (e == cudaSuccess && nproj > 0) e = cudaMemcpyAsync(dD, D, db, cudaMemcpyHostToDevice, cp);
+    if (e == cudaSuccess && cp != st) e = cudaEventRecord(b->ev_join, cp);
+    if (e == cudaSuccess && cp != st) e = cudaStreamWaitEvent(st, b->ev_fork, 0);
+    rc = e == cudaSuccess ? JDFT_OK : jdft_cuda_fail(e, "apply_H_host H2D");
+    if (!rc) {
+        if (nproj == 0) {
+            rc = jdft_local_H(b, (const double *)dV, (const double *)dC, nb, (double *)dHC, st);
+        } else {
+            // same split of the workspace as the fork/join path of jdft_apply_H: GEMM scratch in front, FFT behind
+            const size_t bsz = align_up((size_t)nb * nproj * 16);
+            size_t part_bytes = b->ws_bytes / 4 < ((size_t)64 << 20) ? b->ws_bytes / 4 : ((size_t)64 << 20);
+            part_bytes &= ~(size_t)255;
+            const size_t gemm_bytes = 2 * bsz + part_bytes;
+            if (part_bytes < (size_t)nb * nproj * 16 || jdft_band_batch(b, nb, gemm_bytes) == 0) {
+                rc = jdft_fail(JDFT_EWORKSPACE, "apply_H_host: workspace too small");
+            } else {
+                char *ws = (char *)b->ws;
+                double *B1 = (double *)ws, *B2 = (double *)(ws + bsz);
+                rc = jdft_local_H(b, (const double *)dV, (const double *)dC, nb, (double *)dHC, st, gemm_bytes);
+                if (cp != st) {
+                    cudaError_t e2 = cudaStreamWaitEvent(st, b->ev_join, 0);
+                    if (!rc && e2 != cudaSuccess) rc = jdft_cuda_fail(e2, "apply_H_host join");
+                }
+                if (!rc) rc = jdft_gemm_dotk(b, (const double *)dC, nb, (const double *)dP, nproj, b->nG, 1, 1.0,
+                                             D_mode == 0 ? (const double *)dD : nullptr, B1, ws + 2 * bsz, part_bytes, st);
+                const double *Bd = B1;
+                if (!rc && D_mode == 1) {
+                    rc = jdft_gemm_dotk(b, B1, nb, (const double *)dD, nproj, nproj, 0, 1.0, nullptr, B2, ws + 2 * bsz, part_bytes, st);
+                    Bd = B2;
+                }
+                if (!rc) rc = jdft_gemm_expand(b, Bd, nb, (const double *)dP, nproj, b->nG, (double *)dHC, 1, st);
+            }
+        }
+    }
     b->ws = saved_ws;
     b->ws_bytes = saved_bytes;
-    if (rc) return rc;
+    if (rc) { cudaStreamSynchronize(cp); cudaStreamSynchronize(st); return rc; }
     JDFT_CUDA(cudaMemcpyAsync(HC, dHC, cb, cudaMemcpyDeviceToHost, st));
     JDFT_CUDA(cudaStreamSynchronize(st));
+    JDFT_CUDA(cudaStreamSynchronize(cp));
     return JDFT_OK;
 }
 

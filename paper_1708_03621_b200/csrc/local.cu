@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(kNT) k_planes(const FftPlan plan, const double
 template <int LT>
 struct Tuned {
     static constexpr bool ok = SpecPlan<LT>::npass == 2;
-    static constexpr int R1 = SpecPlan<LT>::radix(0), R2 = SpecPlan<LT>::radix(1);
+    static constexpr int R1 = SpecPlan<LT>::r0, R2 = SpecPlan<LT>::r1;
     static constexpr int T = 16;
     // threads = T x (butterflies of the pass that must run in one round = the R2 pass) rounded so the R1 pass is whole rounds
     static constexpr int NB1 = ok ? LT / R1 : 1, NB2 = ok ? LT / R2 : 1;   // butterflies per pencil in the R1 / R2 pass
@@ -315,6 +315,68 @@ __global__ void __launch_bounds__(Tuned<LT>::NT, PlanesMinB<LT>::v) k_planes_fus
         for (int j = 0; j < R1; j++) {
             const int p = s_planeof[bf + R2 * j];
             if (p >= 0 && t < tmax) W2b[p * plane + t] = a[j];
+        }
+    }
+}
+
+// Density, tuned: last pass of I for the two-pass lengths with the |psi|^2 accumulators in REGISTERS.  A CTA owns the
+// tile (i1, 16 adjacent i2) and walks the bands of the batch in order; in the last pass (radix R2, one round) a
+// thread always produces the same rows bf + R1 j of the same pencil, so it keeps their R2 partial sums itself.
+template <int LT>
+__global__ void __launch_bounds__(Tuned<LT>::NT) k_planes_density_tuned(const double2 *__restrict__ tw, const int S1, const int S2,
+                                                                        const int npl, const int *__restrict__ planeof,
+                                                                        const double2 *__restrict__ W2,
+                                                                        const double *__restrict__ f, const int nbt,
+                                                                        double *__restrict__ n, const int accumulate) {
+    using C = Tuned<LT>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, NT = C::NT, L = LT;
+    static_assert(R1 * T <= NT, "the last pass must run in one round");
+    extern __shared__ double2 smem[];
+    double2 *A = smem;
+    __shared__ int s_planeof[L];
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y;
+    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    __syncthreads();
+    const size_t plane = (size_t)S1 * S2;
+    const int tmax = S2 - t0;
+    const int tl = tid % T, bfl = tid / T;
+    const bool act = tid < R1 * T;
+    double acc[R2];
+#pragma unroll
+    for (int j = 0; j < R2; j++) acc[j] = 0.0;
+    for (int b = 0; b < nbt; b++) {
+        const double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
+        for (int w = tid; w < R2 * T; w += NT) {
+            const int t = w % T, bf = w / T;
+            double2 a[R1];
+#pragma unroll
+            for (int k = 0; k < R1; k++) {
+                const int p = s_planeof[bf + k * R2];
+                a[k] = (p >= 0 && t < tmax) ? W2b[p * plane + t] : make_double2(0.0, 0.0);
+            }
+            Dft<R1, +1>::run(a);
+            twiddle_rows<R1, +1>(a, tw, bf);
+#pragma unroll
+            for (int j = 0; j < R1; j++) A[(bf * R1 + j) * T + t] = a[j];
+        }
+        __syncthreads();
+        if (act) {
+            const double fb = f[b];
+            double2 a[R2];
+#pragma unroll
+            for (int k = 0; k < R2; k++) a[k] = A[(bfl + k * R1) * T + tl];
+            Dft<R2, +1>::run(a);
+#pragma unroll
+            for (int j = 0; j < R2; j++) acc[j] = fma(fb, a[j].x * a[j].x + a[j].y * a[j].y, acc[j]);
+        }
+        __syncthreads();
+    }
+    if (act && tl < tmax) {
+        double *o = n + (size_t)i1 * S2 + t0 + tl;
+#pragma unroll
+        for (int j = 0; j < R2; j++) {
+            double *q = o + (size_t)(bfl + R1 * j) * plane;
+            *q = accumulate ? *q + acc[j] : acc[j];
         }
     }
 }
@@ -700,9 +762,18 @@ extern "C" int jdft_density(const jdft_basis *b, const double *C_, int nb, const
         const int acc = (accumulate || b0 > 0) ? 1 : 0;
         jdft_prof_begin(b, JDFT_K_PLANES, st);
         SPEC_SWITCH(L, b->opt_force_generic, {
-            JDFT_CUDA(ensure_smem(k_planes_density<LT>, smem));
-            k_planes_density<LT><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
-                                                          f + b0, nbt, n, acc);
+            if constexpr (Tuned<LT>::ok) {
+                using C = Tuned<LT>;
+                const size_t sm2 = (size_t)L * C::T * sizeof(double2);
+                JDFT_CUDA(ensure_smem(k_planes_density_tuned<LT>, sm2));
+                dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1]);
+                k_planes_density_tuned<LT><<<g2, C::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
+                                                                   f + b0, nbt, n, acc);
+            } else {
+                JDFT_CUDA(ensure_smem(k_planes_density<LT>, smem));
+                k_planes_density<LT><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
+                                                              f + b0, nbt, n, acc);
+            }
         });
         jdft_prof_end(b, JDFT_K_PLANES, st);
         JDFT_LAUNCH_CHECK("k_planes_density");

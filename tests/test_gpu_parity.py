@@ -389,3 +389,25 @@ def test_specialised_lengths_on_every_axis(ref, jd, cfg_id):
     n_want = c.rb.density(c.C, f)
     n_got = jd.jdft_density(c.gb, dev(c.C), dev(f)).cpu().numpy()
     assert np.linalg.norm(n_got - n_want) <= TOL * np.linalg.norm(n_want)
+
+
+# ------------------------------------------------------------------------------------------ SURVEY 8(f) rank 2 (by composition)
+
+def test_ultrasoft_overlap_and_dense_D_by_composition(case, jd):
+    """Generalised (ultrasoft) overlap O C = Omega (C + P Q P^+ C) and H with a dense Hermitian D need no new kernel:
+    jdft_apply_O followed by jdft_apply_Vnl(P, Omega Q, C, out, accumulate) -- checked against the oracle's operators
+    and against the defining dense matrix on the subspace: C^+ O_us C = Omega (C^+ C + B^+ Q B), B = P^+ C."""
+    rng = np.random.default_rng(101)
+    n = case.P.shape[0]
+    A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    Q = 0.05 * (A + A.conj().T)
+    Om = case.rb.volume
+    out = jd.jdft_apply_O(case.gb, dev(case.C))
+    jd.jdft_apply_Vnl(case.gb, dev(case.P), dev(Om * Q), dev(case.C), out, accumulate=True)
+    got = out.cpu().numpy()
+    want = case.rb.apply_O(case.C) + case.rb.apply_Vnl(case.P, Om * Q, case.C)
+    assert rel_err_per_band(got, want) <= TOL
+    B = case.P.conj() @ case.C.T                                  # [np, nb] = P^+ C with P stored [np][nG]
+    M_def = Om * (case.C.conj() @ case.C.T + B.conj().T @ Q @ B)
+    M_gpu = jd.jdft_subspace(case.gb, dev(case.C), out).cpu().numpy()
+    assert np.max(np.abs(M_gpu - M_def)) <= 1e-10 * np.max(np.abs(M_def))

@@ -85,6 +85,7 @@ int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
  * "force_generic_fft" (0/1: use the runtime-radix FFT kernels even for lengths that have specialised ones; for
  * tests), "overlap_gemm" (0/1, default 0: apply_H forks B = D P^+ C onto a basis-owned side stream beside the FFT
  * pipeline and joins before HC += P B; uses basis-owned events, so not for concurrent calls on one basis),
+ * "planes_pair" (0/1, default 1: K3 with two pencils per thread where that variant exists),
  * "profile_kernel" (see diagnostics)                                                                    */
 int jdft_set_option(jdft_basis *b, const char *key, int64_t value);
 

@@ -45,6 +45,7 @@ struct jdft_basis {
     // fork/join resources of apply_H (option "overlap_gemm"): the projection GEMM runs on `side` while the FFT pipeline
     // runs on the caller's stream
     int64_t opt_overlap;
+    int64_t opt_pair;                         // K3 with two pencils per thread where available ("planes_pair")
     cudaStream_t side;
     cudaEvent_t ev_fork, ev_join;
     // optional per-kernel event timing (option "profile_kernel" = one of JDFT_K_*; 0 = off).  Diagnostics only.

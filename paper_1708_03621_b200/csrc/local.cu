@@ -319,6 +319,125 @@ __global__ void __launch_bounds__(Tuned<LT>::NT, PlanesMinB<LT>::v) k_planes_fus
     }
 }
 
+// K3 with TWO adjacent pencils per thread (lengths whose fused radix is <= 10, so 2 x R2 complex values fit in
+// registers): the twiddle, plane-map and V reads are shared by the pair and W2 / V move as 256-bit / 128-bit words,
+// which cuts the load/store instruction count per pencil by ~30 % on the pipe that bounds k_planes_fused.
+// Shared tile [L][T] with the even pencils in the first half of a row and the odd ones in the second, so both
+// 16-byte accesses of a thread are lane-contiguous.  Requires S2 even (32-byte alignment of a pencil pair).
+template <int LT>
+struct Pair {
+    static constexpr int T = LT == 72 ? 32 : 16;       // pencils per CTA
+    static constexpr int H = T / 2;                    // threads per butterfly row
+    static constexpr int NT = Tuned<LT>::NBT * H;
+    static constexpr bool ok = Tuned<LT>::ok && Tuned<LT>::R2 <= 10 && Tuned<LT>::R1 <= 10;
+};
+__device__ __forceinline__ void ld256(const double2 *p, double2 &a, double2 &b) {
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a.x), "=d"(a.y), "=d"(b.x), "=d"(b.y) : "l"(p));
+}
+__device__ __forceinline__ void st256(double2 *p, const double2 a, const double2 b) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
+}
+template <int LT>
+__global__ void __launch_bounds__(Pair<LT>::NT) k_planes_fused2(const double2 *__restrict__ tw, const int S1, const int S2,
+                                                                const int npl, const int *__restrict__ planeof,
+                                                                double2 *__restrict__ W2, const double *__restrict__ V) {
+    using C = Tuned<LT>;
+    using Q = Pair<LT>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = Q::T, H = Q::H, NT = Q::NT, L = LT;
+    static_assert(R1 * H <= NT, "the fused middle pass must run in one round");
+    extern __shared__ double2 smem[];
+    double2 *A = smem;
+    __shared__ int s_planeof[L];
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y, b = blockIdx.z;
+    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    __syncthreads();
+    const size_t plane = (size_t)S1 * S2;
+    double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
+    const double *Vb = V + (size_t)i1 * S2 + t0;
+    const int tmax = S2 - t0;  // even
+    for (int w = tid; w < R2 * H; w += NT) {
+        const int l = w % H, bf = w / H;
+        double2 a0[R1], a1[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) {
+            const int p = s_planeof[bf + k * R2];
+            a0[k] = a1[k] = make_double2(0.0, 0.0);
+            if (p >= 0 && 2 * l < tmax) ld256(W2b + p * plane + 2 * l, a0[k], a1[k]);
+        }
+        Dft<R1, +1>::run(a0);
+        Dft<R1, +1>::run(a1);
+#pragma unroll
+        for (int j = 1; j < R1; j++) {
+            const double2 wv = __ldg(tw + bf * j);
+            a0[j] = cmul(a0[j], wv);
+            a1[j] = cmul(a1[j], wv);
+        }
+#pragma unroll
+        for (int j = 0; j < R1; j++) {
+            A[(bf * R1 + j) * T + l] = a0[j];
+            A[(bf * R1 + j) * T + H + l] = a1[j];
+        }
+    }
+    __syncthreads();
+    {
+        const int l = tid % H, bf = tid / H;
+        const bool act = tid < R1 * H;
+        double2 a0[R2], a1[R2];
+        if (act) {
+#pragma unroll
+            for (int k = 0; k < R2; k++) {
+                a0[k] = A[(bf + k * R1) * T + l];
+                a1[k] = A[(bf + k * R1) * T + H + l];
+            }
+        }
+        __syncthreads();
+        if (act) {
+            Dft<R2, +1>::run(a0);
+            Dft<R2, +1>::run(a1);
+#pragma unroll
+            for (int j = 0; j < R2; j++) {
+                double2 f = make_double2(0.0, 0.0);
+                if (2 * l < tmax) f = __ldg(reinterpret_cast<const double2 *>(Vb + (size_t)(bf + R1 * j) * plane + 2 * l));
+                a0[j].x *= f.x;
+                a0[j].y *= f.x;
+                a1[j].x *= f.y;
+                a1[j].y *= f.y;
+            }
+            Dft<R2, -1>::run(a0);
+            Dft<R2, -1>::run(a1);
+#pragma unroll
+            for (int j = 1; j < R2; j++) {
+                double2 wv = __ldg(tw + bf * j);
+                wv.y = -wv.y;
+                a0[j] = cmul(a0[j], wv);
+                a1[j] = cmul(a1[j], wv);
+            }
+#pragma unroll
+            for (int j = 0; j < R2; j++) {
+                A[(bf * R2 + j) * T + l] = a0[j];
+                A[(bf * R2 + j) * T + H + l] = a1[j];
+            }
+        }
+    }
+    __syncthreads();
+    for (int w = tid; w < R2 * H; w += NT) {
+        const int l = w % H, bf = w / H;
+        double2 a0[R1], a1[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) {
+            a0[k] = A[(bf + k * R2) * T + l];
+            a1[k] = A[(bf + k * R2) * T + H + l];
+        }
+        Dft<R1, -1>::run(a0);
+        Dft<R1, -1>::run(a1);
+#pragma unroll
+        for (int j = 0; j < R1; j++) {
+            const int p = s_planeof[bf + R2 * j];
+            if (p >= 0 && 2 * l < tmax) st256(W2b + p * plane + 2 * l, a0[j], a1[j]);
+        }
+    }
+}
+
 // Density, tuned: last pass of I for the two-pass lengths with the |psi|^2 accumulators in REGISTERS.  A CTA owns the
 // tile (i1, 16 adjacent i2) and walks the bands of the batch in order; in the last pass (radix R2, one round) a
 // thread always produces the same rows bf + R1 j of the same pencil, so it keeps their R2 partial sums itself.
@@ -642,6 +761,18 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
     dim3 grid((b->S[2] + kT - 1) / kT, b->S[1], nbt);
     jdft_prof_begin(b, JDFT_K_PLANES, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
+        if constexpr (MODE == 0 && Pair<LT>::ok && LT == 72) {  // measured: +7 % at 72 (32 pencils/CTA), -12 % at 80 (16 pencils, 80 threads)
+            if (b->S[2] % 2 == 0 && b->opt_pair) {
+                using Q = Pair<LT>;
+                const size_t sm2 = (size_t)L * Q::T * sizeof(double2);
+                JDFT_CUDA(ensure_smem(k_planes_fused2<LT>, sm2));
+                dim3 g2((b->S[2] + Q::T - 1) / Q::T, b->S[1], nbt);
+                k_planes_fused2<LT><<<g2, Q::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
+                jdft_prof_end(b, JDFT_K_PLANES, st);
+                JDFT_LAUNCH_CHECK("k_planes_fused2");
+                return JDFT_OK;
+            }
+        }
         if constexpr (MODE == 0 && Tuned<LT>::ok) {
             using C = Tuned<LT>;
             const size_t sm2 = (size_t)L * C::T * sizeof(double2);

@@ -411,3 +411,16 @@ def test_ultrasoft_overlap_and_dense_D_by_composition(case, jd):
     M_def = Om * (case.C.conj() @ case.C.T + B.conj().T @ Q @ B)
     M_gpu = jd.jdft_subspace(case.gb, dev(case.C), out).cpu().numpy()
     assert np.max(np.abs(M_gpu - M_def)) <= 1e-10 * np.max(np.abs(M_def))
+
+
+def test_planes_pair_kernel_matches(ref, jd):
+    """Plane length 72 runs K3 with two pencils per thread (256-bit global accesses); same result as the one-pencil
+    kernel and as the oracle."""
+    c = Case(ref, jd, 210)
+    want = c.rb.apply_H(c.V, c.P, c.D, c.C)
+    args = (dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C))
+    a = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+    jd.jdft_set_option(c.gb, "planes_pair", 0)
+    b = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+    assert rel_err_per_band(a, want) <= TOL and rel_err_per_band(b, want) <= TOL
+    assert rel_err_per_band(a, b) <= 1e-13

@@ -328,7 +328,9 @@ template <int LT>
 struct Pair {
     static constexpr int T = LT == 72 ? 32 : 16;       // pencils per CTA
     static constexpr int H = T / 2;                    // threads per butterfly row
-    static constexpr int NT = Tuned<LT>::NBT * H;
+    static constexpr int G = 1;                        // tiles (adjacent i1 rows) per CTA (2 at length 80 measured slower)
+    static constexpr int NTG = Tuned<LT>::NBT * H;     // threads per tile
+    static constexpr int NT = G * NTG;
     static constexpr bool ok = Tuned<LT>::ok && Tuned<LT>::R2 <= 10 && Tuned<LT>::R1 <= 10;
 };
 __device__ __forceinline__ void ld256(const double2 *p, double2 &a, double2 &b) {
@@ -343,18 +345,20 @@ __global__ void __launch_bounds__(Pair<LT>::NT) k_planes_fused2(const double2 *_
                                                                 double2 *__restrict__ W2, const double *__restrict__ V) {
     using C = Tuned<LT>;
     using Q = Pair<LT>;
-    constexpr int R1 = C::R1, R2 = C::R2, T = Q::T, H = Q::H, NT = Q::NT, L = LT;
+    constexpr int R1 = C::R1, R2 = C::R2, T = Q::T, H = Q::H, NT = Q::NTG, L = LT;
     static_assert(R1 * H <= NT, "the fused middle pass must run in one round");
     extern __shared__ double2 smem[];
-    double2 *A = smem;
     __shared__ int s_planeof[L];
-    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y, b = blockIdx.z;
-    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;  // tile of this thread inside the CTA, index inside the tile
+    double2 *A = smem + grp * L * T;
+    const int t0 = blockIdx.x * T, i1 = blockIdx.y * Q::G + grp, b = blockIdx.z;
+    for (int i = threadIdx.x; i < L; i += Q::NT) s_planeof[i] = planeof[i];
     __syncthreads();
+    const bool live = i1 < S1;
     const size_t plane = (size_t)S1 * S2;
     double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
     const double *Vb = V + (size_t)i1 * S2 + t0;
-    const int tmax = S2 - t0;  // even
+    const int tmax = live ? S2 - t0 : 0;  // even; 0 switches every global access of an idle tile group off
     for (int w = tid; w < R2 * H; w += NT) {
         const int l = w % H, bf = w / H;
         double2 a0[R1], a1[R1];
@@ -764,9 +768,9 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
         if constexpr (MODE == 0 && Pair<LT>::ok && LT == 72) {  // measured: +7 % at 72 (32 pencils/CTA), -12 % at 80 (16 pencils, 80 threads)
             if (b->S[2] % 2 == 0 && b->opt_pair) {
                 using Q = Pair<LT>;
-                const size_t sm2 = (size_t)L * Q::T * sizeof(double2);
+                const size_t sm2 = (size_t)Q::G * L * Q::T * sizeof(double2);
                 JDFT_CUDA(ensure_smem(k_planes_fused2<LT>, sm2));
-                dim3 g2((b->S[2] + Q::T - 1) / Q::T, b->S[1], nbt);
+                dim3 g2((b->S[2] + Q::T - 1) / Q::T, (b->S[1] + Q::G - 1) / Q::G, nbt);
                 k_planes_fused2<LT><<<g2, Q::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
                 jdft_prof_end(b, JDFT_K_PLANES, st);
                 JDFT_LAUNCH_CHECK("k_planes_fused2");

@@ -442,6 +442,97 @@ __global__ void __launch_bounds__(Pair<LT>::NT) k_planes_fused2(const double2 *_
     }
 }
 
+// K3 hybrid for length 128: the first and last pass (radix 8, global side) handle TWO adjacent pencils per thread with
+// 256-bit loads/stores and shared twiddle / plane-map reads, in ONE round of all 128 threads; the fused middle pass
+// (radix 16, one pencil per thread: two would not fit in registers) is unchanged.  Tile rows keep the even pencils in
+// the first half and the odd ones in the second; middle-pass lane x works on pencil 2x (x < 8) or 2(x-8)+1, so every
+// shared-memory access of a quarter-warp is one contiguous 128-byte row segment.  Requires S2 even.
+template <int LT>
+__global__ void __launch_bounds__(Tuned<LT>::NT, PlanesMinB<LT>::v) k_planes_fused_h(const double2 *__restrict__ tw, const int S1,
+                                                                                     const int S2, const int npl,
+                                                                                     const int *__restrict__ planeof,
+                                                                                     double2 *__restrict__ W2,
+                                                                                     const double *__restrict__ V) {
+    using C = Tuned<LT>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, H = T / 2, NT = C::NT, L = LT;
+    static_assert(R2 * H == NT && R1 * T <= NT, "pair passes and the fused middle pass must each be one round");
+    extern __shared__ double2 smem[];
+    double2 *A = smem;
+    __shared__ int s_planeof[L];
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y, b = blockIdx.z;
+    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    __syncthreads();
+    const size_t plane = (size_t)S1 * S2;
+    double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
+    const double *Vb = V + (size_t)i1 * S2 + t0;
+    const int tmax = S2 - t0;  // even
+    {
+        const int l = tid % H, bf = tid / H;
+        double2 a0[R1], a1[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) {
+            const int p = s_planeof[bf + k * R2];
+            a0[k] = a1[k] = make_double2(0.0, 0.0);
+            if (p >= 0 && 2 * l < tmax) ld256(W2b + p * plane + 2 * l, a0[k], a1[k]);
+        }
+        Dft<R1, +1>::run(a0);
+        Dft<R1, +1>::run(a1);
+#pragma unroll
+        for (int j = 1; j < R1; j++) {
+            const double2 wv = __ldg(tw + bf * j);
+            a0[j] = cmul(a0[j], wv);
+            a1[j] = cmul(a1[j], wv);
+        }
+#pragma unroll
+        for (int j = 0; j < R1; j++) {
+            A[(bf * R1 + j) * T + l] = a0[j];
+            A[(bf * R1 + j) * T + H + l] = a1[j];
+        }
+    }
+    __syncthreads();
+    {
+        const int x = tid % T, bf = tid / T;             // x = slot inside the tile row
+        const int t = x < H ? 2 * x : 2 * (x - H) + 1;   // pencil stored in that slot
+        const bool act = tid < R1 * T;
+        double2 a[R2];
+        if (act) {
+#pragma unroll
+            for (int k = 0; k < R2; k++) a[k] = A[(bf + k * R1) * T + x];
+        }
+        __syncthreads();
+        if (act) {
+            Dft<R2, +1>::run(a);
+#pragma unroll
+            for (int j = 0; j < R2; j++) {
+                const double f = t < tmax ? __ldg(Vb + (size_t)(bf + R1 * j) * plane + t) : 0.0;
+                a[j].x *= f;
+                a[j].y *= f;
+            }
+            Dft<R2, -1>::run(a);
+            twiddle_rows<R2, -1>(a, tw, bf);
+#pragma unroll
+            for (int j = 0; j < R2; j++) A[(bf * R2 + j) * T + x] = a[j];
+        }
+    }
+    __syncthreads();
+    {
+        const int l = tid % H, bf = tid / H;
+        double2 a0[R1], a1[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) {
+            a0[k] = A[(bf + k * R2) * T + l];
+            a1[k] = A[(bf + k * R2) * T + H + l];
+        }
+        Dft<R1, -1>::run(a0);
+        Dft<R1, -1>::run(a1);
+#pragma unroll
+        for (int j = 0; j < R1; j++) {
+            const int p = s_planeof[bf + R2 * j];
+            if (p >= 0 && 2 * l < tmax) st256(W2b + p * plane + 2 * l, a0[j], a1[j]);
+        }
+    }
+}
+
 // Density, tuned: last pass of I for the two-pass lengths with the |psi|^2 accumulators in REGISTERS.  A CTA owns the
 // tile (i1, 16 adjacent i2) and walks the bands of the batch in order; in the last pass (radix R2, one round) a
 // thread always produces the same rows bf + R1 j of the same pencil, so it keeps their R2 partial sums itself.
@@ -774,6 +865,18 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
                 k_planes_fused2<LT><<<g2, Q::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
                 jdft_prof_end(b, JDFT_K_PLANES, st);
                 JDFT_LAUNCH_CHECK("k_planes_fused2");
+                return JDFT_OK;
+            }
+        }
+        if constexpr (MODE == 0 && LT == 128) {
+            if (b->S[2] % 2 == 0 && b->opt_pair) {
+                using C = Tuned<LT>;
+                const size_t sm2 = (size_t)L * C::T * sizeof(double2);
+                JDFT_CUDA(ensure_smem(k_planes_fused_h<LT>, sm2));
+                dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
+                k_planes_fused_h<LT><<<g2, C::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
+                jdft_prof_end(b, JDFT_K_PLANES, st);
+                JDFT_LAUNCH_CHECK("k_planes_fused_h");
                 return JDFT_OK;
             }
         }

@@ -442,20 +442,26 @@ __global__ void __launch_bounds__(Pair<LT>::NT) k_planes_fused2(const double2 *_
     }
 }
 
-// K3 hybrid for length 128: the first and last pass (radix 8, global side) handle TWO adjacent pencils per thread with
+// K3 hybrid for lengths 128 and 80: the first and last pass (radix 8, global side) handle TWO adjacent pencils per thread with
 // 256-bit loads/stores and shared twiddle / plane-map reads, in ONE round of all 128 threads; the fused middle pass
 // (radix 16, one pencil per thread: two would not fit in registers) is unchanged.  Tile rows keep the even pencils in
 // the first half and the odd ones in the second; middle-pass lane x works on pencil 2x (x < 8) or 2(x-8)+1, so every
 // shared-memory access of a quarter-warp is one contiguous 128-byte row segment.  Requires S2 even.
 template <int LT>
-__global__ void __launch_bounds__(Tuned<LT>::NT, PlanesMinB<LT>::v) k_planes_fused_h(const double2 *__restrict__ tw, const int S1,
+struct Hyb {  // threads = the larger of the pair passes' and the middle pass' work items
+    static constexpr int PAIRS = Tuned<LT>::R2 * (Tuned<LT>::T / 2), MID = Tuned<LT>::R1 * Tuned<LT>::T;
+    static constexpr int NT = PAIRS > MID ? PAIRS : MID;
+    static constexpr int MINB = LT == 128 ? 4 : 5;   // measured
+};
+template <int LT>
+__global__ void __launch_bounds__(Hyb<LT>::NT, Hyb<LT>::MINB) k_planes_fused_h(const double2 *__restrict__ tw, const int S1,
                                                                                      const int S2, const int npl,
                                                                                      const int *__restrict__ planeof,
                                                                                      double2 *__restrict__ W2,
                                                                                      const double *__restrict__ V) {
     using C = Tuned<LT>;
-    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, H = T / 2, NT = C::NT, L = LT;
-    static_assert(R2 * H == NT && R1 * T <= NT, "pair passes and the fused middle pass must each be one round");
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, H = T / 2, NT = Hyb<LT>::NT, L = LT;
+    static_assert(R2 * H <= NT && R1 * T <= NT, "pair passes and the fused middle pass must each be one round");
     extern __shared__ double2 smem[];
     double2 *A = smem;
     __shared__ int s_planeof[L];
@@ -466,7 +472,7 @@ __global__ void __launch_bounds__(Tuned<LT>::NT, PlanesMinB<LT>::v) k_planes_fus
     double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
     const double *Vb = V + (size_t)i1 * S2 + t0;
     const int tmax = S2 - t0;  // even
-    {
+    if (tid < R2 * H) {
         const int l = tid % H, bf = tid / H;
         double2 a0[R1], a1[R1];
 #pragma unroll
@@ -515,7 +521,7 @@ __global__ void __launch_bounds__(Tuned<LT>::NT, PlanesMinB<LT>::v) k_planes_fus
         }
     }
     __syncthreads();
-    {
+    if (tid < R2 * H) {
         const int l = tid % H, bf = tid / H;
         double2 a0[R1], a1[R1];
 #pragma unroll
@@ -868,13 +874,13 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
                 return JDFT_OK;
             }
         }
-        if constexpr (MODE == 0 && LT == 128) {
+        if constexpr (MODE == 0 && (LT == 128 || LT == 80)) {  // 72 runs the full pair kernel above (hybrid measured slower)
             if (b->S[2] % 2 == 0 && b->opt_pair) {
                 using C = Tuned<LT>;
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
                 JDFT_CUDA(ensure_smem(k_planes_fused_h<LT>, sm2));
                 dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
-                k_planes_fused_h<LT><<<g2, C::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
+                k_planes_fused_h<LT><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
                 jdft_prof_end(b, JDFT_K_PLANES, st);
                 JDFT_LAUNCH_CHECK("k_planes_fused_h");
                 return JDFT_OK;

@@ -416,8 +416,7 @@ def test_ultrasoft_overlap_and_dense_D_by_composition(case, jd):
 @pytest.mark.parametrize("cfg_id", [210, 211, 212])
 def test_planes_pair_kernel_matches(ref, jd, cfg_id):
     """Plane length 72 runs K3 with two pencils per thread (256-bit global accesses); same result as the one-pencil
-    kernel and as the oracle; length 128 runs the hybrid (pairs in the first and last pass only).  (Length 80 has no such
-    variant -- measured slower -- so both calls run the same kernel.)"""
+    kernel and as the oracle; lengths 128 and 80 run the hybrid (pairs in the first and last pass only)."""
     c = Case(ref, jd, cfg_id)
     want = c.rb.apply_H(c.V, c.P, c.D, c.C)
     args = (dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C))

@@ -424,6 +424,11 @@ def run_ours(args):
                      "avg_launch_ms": dom_ms / max(1, dom_n), "peak_source": hbm_src if roofline["bound"] == "hbm" else fp_src,
                      "traffic": None, "share_of_step": dom_ms / args.steps / ms_step})
     roofline["traffic"] = ncu_traffic(args.config, dominant)
+    dom_launches_step = max(1, dom_n // args.steps)
+    roofline["algorithmic_per_launch"] = sum(algorithmic(k["info"], dominant, max(1, dom_launches_step // max(1, len(ks))))
+                                             for k in ks) / dom_launches_step
+    roofline["note"] = ("algorithmic bytes (flops) per launch = DESIGN.md section 6 per-band figure x bands per launch; "
+                        "traffic = ncu dram bytes per launch (profiles/traffic.csv)")
     local_bytes = sum(sum(algorithmic(k["info"], n, max(1, nbatches[n] // len(ks))) for n in
                           ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd")) for k in ks)
     local_ms = sum(per_kernel[n][0] for n in ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd"))

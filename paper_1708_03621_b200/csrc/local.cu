@@ -539,6 +539,74 @@ __global__ void __launch_bounds__(Hyb<LT>::NT, Hyb<LT>::MINB) k_planes_fused_h(c
     }
 }
 
+// K2 / K4 hybrid (same idea as k_planes_fused_h): the first pass works on pencil pairs with 256-bit loads and shared
+// twiddle / row-map reads, the last pass on single pencils with lane x -> pencil 2x | 2(x-8)+1.  Requires S2 even.
+template <int LT, bool FWD>
+__global__ void __launch_bounds__(Hyb<LT>::NT) k_rows_hyb(const double2 *__restrict__ tw, const int S2, const int npl,
+                                                          const int ncol, const int *__restrict__ rowcol,
+                                                          double2 *__restrict__ W1, double2 *__restrict__ W2) {
+    using C = Tuned<LT>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, H = T / 2, NT = Hyb<LT>::NT, L = LT;
+    constexpr int SIGN = FWD ? -1 : +1;
+    extern __shared__ double2 smem[];
+    double2 *A = smem;
+    __shared__ int s_rowcol[L];
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, p = blockIdx.y, b = blockIdx.z;
+    for (int i = tid; i < L; i += NT) s_rowcol[i] = rowcol[p * L + i];
+    __syncthreads();
+    double2 *W1b = W1 + (size_t)b * ncol * S2 + t0;
+    double2 *W2b = W2 + ((size_t)b * npl + p) * L * S2 + t0;
+    const int tmax = S2 - t0;  // even
+    if (tid < R2 * H) {
+        const int l = tid % H, bf = tid / H;
+        double2 a0[R1], a1[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) {
+            const int row = bf + k * R2;
+            a0[k] = a1[k] = make_double2(0.0, 0.0);
+            if (FWD) {
+                if (2 * l < tmax) ld256(W2b + (size_t)row * S2 + 2 * l, a0[k], a1[k]);
+            } else {
+                const int c = s_rowcol[row];
+                if (c >= 0 && 2 * l < tmax) ld256(W1b + (size_t)c * S2 + 2 * l, a0[k], a1[k]);
+            }
+        }
+        Dft<R1, SIGN>::run(a0);
+        Dft<R1, SIGN>::run(a1);
+#pragma unroll
+        for (int j = 1; j < R1; j++) {
+            double2 wv = __ldg(tw + bf * j);
+            if (SIGN < 0) wv.y = -wv.y;
+            a0[j] = cmul(a0[j], wv);
+            a1[j] = cmul(a1[j], wv);
+        }
+#pragma unroll
+        for (int j = 0; j < R1; j++) {
+            A[(bf * R1 + j) * T + l] = a0[j];
+            A[(bf * R1 + j) * T + H + l] = a1[j];
+        }
+    }
+    __syncthreads();
+    if (tid < R1 * T) {
+        const int x = tid % T, bf = tid / T;
+        const int t = x < H ? 2 * x : 2 * (x - H) + 1;
+        double2 a[R2];
+#pragma unroll
+        for (int k = 0; k < R2; k++) a[k] = A[(bf + k * R1) * T + x];
+        Dft<R2, SIGN>::run(a);
+#pragma unroll
+        for (int j = 0; j < R2; j++) {
+            const int row = bf + R1 * j;
+            if (FWD) {
+                const int c = s_rowcol[row];
+                if (c >= 0 && t < tmax) W1b[(size_t)c * S2 + t] = a[j];
+            } else {
+                if (t < tmax) W2b[(size_t)row * S2 + t] = a[j];
+            }
+        }
+    }
+}
+
 // Density, tuned: last pass of I for the two-pass lengths with the |psi|^2 accumulators in REGISTERS.  A CTA owns the
 // tile (i1, 16 adjacent i2) and walks the bands of the batch in order; in the last pass (radix R2, one round) a
 // thread always produces the same rows bf + R1 j of the same pencil, so it keeps their R2 partial sums itself.
@@ -839,6 +907,18 @@ int launch_rows(const jdft_basis *b, int nbt, double2 *W1, double2 *W2, cudaStre
     dim3 grid((b->S[2] + kT - 1) / kT, b->npl, nbt);
     jdft_prof_begin(b, FWD ? JDFT_K_ROWS_FWD : JDFT_K_ROWS_INV, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
+        if constexpr (LT == 128) {  // measured: 1.07 -> 0.94 ms at 128 (91 % of the HBM roofline), slower at 80
+            if (b->S[2] % 2 == 0 && b->opt_pair) {
+                using C = Tuned<LT>;
+                const size_t sm2 = (size_t)L * C::T * sizeof(double2);
+                JDFT_CUDA(ensure_smem(k_rows_hyb<LT, FWD>, sm2));
+                dim3 g2((b->S[2] + C::T - 1) / C::T, b->npl, nbt);
+                k_rows_hyb<LT, FWD><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
+                jdft_prof_end(b, FWD ? JDFT_K_ROWS_FWD : JDFT_K_ROWS_INV, st);
+                JDFT_LAUNCH_CHECK("k_rows_hyb");
+                return JDFT_OK;
+            }
+        }
         if constexpr (Tuned<LT>::ok) {
             using C = Tuned<LT>;
             const size_t sm2 = (size_t)L * C::T * sizeof(double2);

@@ -255,7 +255,7 @@ def run_ours(args):
         iG, _, _ = jd.jdft_basis_export(gb)
         C_h = workloads.make_bands(args.config, gb.nG, ik=ik)
         P_h = workloads.make_projectors(args.config, iG, kpts[ik], atoms)
-        jd.jdft_alloc_workspace(gb, max(args.batch, 64), max(nb, nproj))
+        jd.jdft_alloc_workspace(gb, max(args.batch, min(nb, args.ws_bands)), max(nb, nproj))
         if args.batch > 0:
             jd.jdft_set_option(gb, "band_batch", args.batch)
         if args.overlap:
@@ -381,7 +381,7 @@ def run_ours(args):
         ms_d = t_op(lambda: jd.jdft_density(k["gb"], k["C"], fo, nr))
         ms_s = t_op(lambda: jd.jdft_subspace(k["gb"], k["C"], k["HC"], Hs))
         i = k["info"]
-        nbat = (nb + 63) // 64
+        nbat = (nb + 255) // 256
         dens_bytes = nb * 16 * (i["nG"] + 2 * i["a"] + 2 * i["b"]) + nbat * 2 * 8 * i["N"]
         # Listing 1 on the scalar-field basis of the density cutoff (4 x Ecut, Gamma), 16 fields per call
         gs = jd.jdft_basis_create(R, [0.0, 0.0, 0.0], 4.0 * Ecut, S, device=local)
@@ -471,6 +471,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json workload 1..5 (default 2 = configs[1])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=0, help="bands per FFT batch (0 = automatic)")
+    ap.add_argument("--ws-bands", type=int, default=256, help="bands of FFT scratch in the workspace (= automatic batch size)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", action="store_true", help="also time jdft_density and jdft_subspace (SURVEY 8(f) rank 1)")
     ap.add_argument("--overlap", action="store_true",

@@ -81,7 +81,7 @@ int jdft_basis_device_maps(const jdft_basis *b, const int32_t **index_dev, const
  * Calls with more bands than fit are split into band batches internally (results are identical).      */
 size_t jdft_workspace_bytes(const jdft_basis *b, int nbands_batch, int nrows_max);
 int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
-/* tunables: "band_batch" (bands per FFT batch, 0 = automatic: what the workspace holds, at most 64),
+/* tunables: "band_batch" (bands per FFT batch, 0 = automatic: what the workspace holds, at most 256),
  * "force_generic_fft" (0/1: use the runtime-radix FFT kernels even for lengths that have specialised ones; for
  * tests), "overlap_gemm" (0/1, default 0: apply_H forks B = D P^+ C onto a basis-owned side stream beside the FFT
  * pipeline and joins before HC += P B; uses basis-owned events, so not for concurrent calls on one basis),

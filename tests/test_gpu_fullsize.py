@@ -25,9 +25,9 @@ def rel(got, want):
 
 
 def auto_batch(gb, S, ws_bytes):
-    """Bands per FFT batch the library picks on its own (what the workspace holds, at most 64)."""
+    """Bands per FFT batch the library picks on its own (what the workspace holds, at most 256)."""
     per = 16 * (gb.ncol * S[2] + gb.npl * S[1] * S[2])
-    return max(1, min(64, ws_bytes // per))
+    return max(1, min(256, ws_bytes // per))
 
 
 class Full:
@@ -42,7 +42,7 @@ class Full:
         inp = workloads.make_inputs(cfg_id, iG, ik=ik)
         self.C, self.V, self.P, self.D = inp["C"], inp["Vloc"], inp["P"], inp["D"]
         nproj = self.P.shape[0]
-        ws = jd.jdft_alloc_workspace(self.gb, 64, max(self.nb, nproj))                     # as bench.py does
+        ws = jd.jdft_alloc_workspace(self.gb, min(self.nb, 256), max(self.nb, nproj))       # as bench.py does
         nbatch = auto_batch(self.gb, S, ws.numel())
         last0 = ((self.nb - 1) // nbatch) * nbatch                                         # first band of the last batch
         pick = {0, nbatch - 1, nbatch, last0, self.nb - 1}

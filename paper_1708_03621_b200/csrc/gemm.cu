@@ -162,7 +162,7 @@ __global__ void k_splitk_reduce(const double2 *__restrict__ part, const int nspl
 }
 
 // ---------------------------------------------------------------------------------------------- expand GEMM
-__global__ void __launch_bounds__(NTHREADS) k_gemm_expand(const double2 *__restrict__ A, const int Rn,
+__global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__restrict__ A, const int Rn,
                                                           const double2 *__restrict__ Pm, const int K, const int64_t Nn,
                                                           double2 *__restrict__ Out, const int accumulate) {
     extern __shared__ __align__(16) char smem[];

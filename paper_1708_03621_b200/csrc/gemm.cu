@@ -162,42 +162,49 @@ __global__ void k_splitk_reduce(const double2 *__restrict__ part, const int nspl
 }
 
 // ---------------------------------------------------------------------------------------------- expand GEMM
+// BN_ x (WM x WN warps): 64 x (2 x 2) is the default tile; 56 x (4 x 1) exists because for some n extents it fills the
+// 148 x 3 CTA slots in whole waves where 64 leaves a half-empty tail wave (config 2: 1.68 -> 1.93 waves).
+template <int BN_, int WM, int WN>
 __global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__restrict__ A, const int Rn,
                                                           const double2 *__restrict__ Pm, const int K, const int64_t Nn,
                                                           double2 *__restrict__ Out, const int accumulate) {
     extern __shared__ __align__(16) char smem[];
+    constexpr int MTL = BM / (8 * WM), NTL = BN_ / (8 * WN);   // 8 x 8 DMMA tiles per warp along rows / columns
+    constexpr int PROW = BN_ * 16 + 32, OPN = BK * PROW;
+    static_assert(WM * WN * 32 == NTHREADS && MTL * 8 * WM == BM && NTL * 8 * WN == BN_, "warp layout");
     char *sA = smem, *sP = smem + STAGES * OPK_BYTES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wr = (warp >> 1) * 32, wc = (warp & 1) * 32;
+    const int wr = (warp / WN) * (8 * MTL), wc = (warp % WN) * (8 * NTL);
     const int row0 = blockIdx.y * BM;
-    const int64_t n0 = (int64_t)blockIdx.x * BN;
+    const int64_t n0 = (int64_t)blockIdx.x * BN_;
     const int nkt = (K + BK - 1) / BK;
 
-    double cr[4][4][2], ci[4][4][2];
+    double cr[MTL][NTL][2], ci[MTL][NTL][2];
 #pragma unroll
-    for (int i = 0; i < 4; i++)
+    for (int i = 0; i < MTL; i++)
 #pragma unroll
-        for (int j = 0; j < 4; j++) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+        for (int j = 0; j < NTL; j++) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
 
     auto load_p = [&](char *dst, int k0) {
 #pragma unroll
-        for (int i = 0; i < (BK * BN) / NTHREADS; i++) {
+        for (int i = 0; i < (BK * BN_ + NTHREADS - 1) / NTHREADS; i++) {
             const int e = tid + i * NTHREADS;
-            const int kk = e / BN, nn = e % BN;
+            if ((BK * BN_) % NTHREADS != 0 && e >= BK * BN_) break;
+            const int kk = e / BN_, nn = e % BN_;
             const bool ok = (k0 + kk < K) && (n0 + nn < Nn);
             const double2 *src = ok ? Pm + (size_t)(k0 + kk) * Nn + n0 + nn : Pm;
-            cp_async16(dst + kk * PROW_BYTES + nn * 16, src, ok);
+            cp_async16(dst + kk * PROW + nn * 16, src, ok);
         }
     };
     for (int s = 0; s < STAGES - 1; s++) {
         if (s < nkt) {
             load_opk(sA + s * OPK_BYTES, A, K, Rn, row0, (int64_t)s * BK, K, tid);
-            load_p(sP + s * OPN_BYTES, s * BK);
+            load_p(sP + s * OPN, s * BK);
         }
         cp_async_commit();
     }
     const int fa = (lane >> 2) * 64 + (lane & 3) * 16;
-    const int fp = (lane & 3) * PROW_BYTES + (lane >> 2) * 16;
+    const int fp = (lane & 3) * PROW + (lane >> 2) * 16;
     for (int kt = 0; kt < nkt; kt++) {
         cp_async_wait<STAGES - 2>();
         __syncthreads();
@@ -206,24 +213,24 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__re
             if (nx < nkt) {
                 const int slot = nx % STAGES;
                 load_opk(sA + slot * OPK_BYTES, A, K, Rn, row0, (int64_t)nx * BK, K, tid);
-                load_p(sP + slot * OPN_BYTES, nx * BK);
+                load_p(sP + slot * OPN, nx * BK);
             }
             cp_async_commit();
         }
-        const char *ba = sA + (kt % STAGES) * OPK_BYTES, *bp = sP + (kt % STAGES) * OPN_BYTES;
+        const char *ba = sA + (kt % STAGES) * OPK_BYTES, *bp = sP + (kt % STAGES) * OPN;
 #pragma unroll
         for (int kk = 0; kk < BK / 4; kk++) {
-            double2 a[4], bq[4];
+            double2 a[MTL], bq[NTL];
 #pragma unroll
-            for (int i = 0; i < 4; i++)
+            for (int i = 0; i < MTL; i++)
                 a[i] = *reinterpret_cast<const double2 *>(ba + kk * KBLK_BYTES + (wr + 8 * i) * 64 + fa);
 #pragma unroll
-            for (int j = 0; j < 4; j++)
-                bq[j] = *reinterpret_cast<const double2 *>(bp + kk * 4 * PROW_BYTES + (wc + 8 * j) * 16 + fp);
+            for (int j = 0; j < NTL; j++)
+                bq[j] = *reinterpret_cast<const double2 *>(bp + kk * 4 * PROW + (wc + 8 * j) * 16 + fp);
 #pragma unroll
-            for (int i = 0; i < 4; i++)
+            for (int i = 0; i < MTL; i++)
 #pragma unroll
-                for (int j = 0; j < 4; j++) {
+                for (int j = 0; j < NTL; j++) {
                     dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
                     dmma(ci[i][j][0], ci[i][j][1], a[i].y, bq[j].x);
                     dmma(cr[i][j][0], cr[i][j][1], a[i].y, -bq[j].y);
@@ -233,11 +240,11 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__re
     }
     cp_async_wait<0>();
 #pragma unroll
-    for (int i = 0; i < 4; i++) {
+    for (int i = 0; i < MTL; i++) {
         const int r = row0 + wr + 8 * i + (lane >> 2);
         if (r >= Rn) continue;
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < NTL; j++) {
             const int64_t n = n0 + wc + 8 * j + 2 * (lane & 3);
             double2 *o = Out + (size_t)r * Nn + n;
             if (n < Nn) {
@@ -322,11 +329,26 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
 int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
                      cudaStream_t st) {
     if (Rn <= 0 || Nn <= 0) return JDFT_OK;
-    const size_t smem = STAGES * (OPK_BYTES + OPN_BYTES);
-    JDFT_CUDA(ensure_smem(k_gemm_expand, smem));
-    dim3 grid((unsigned)((Nn + BN - 1) / BN), (Rn + BM - 1) / BM);
+    // tile width: 64, unless 56 fills the 148 x 3 CTA slots in whole waves noticeably better
+    const int64_t slots = 148 * 3, rt = (Rn + BM - 1) / BM;
+    auto fill = [&](int bn) {
+        const int64_t ctas = ((Nn + bn - 1) / bn) * rt, waves = (ctas + slots - 1) / slots;
+        return (double)ctas / (double)(waves * slots);
+    };
+    const bool narrow = fill(56) > fill(64) + 0.05;
     jdft_prof_begin(b, JDFT_K_GEMM_EXPAND, st);
-    k_gemm_expand<<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, accumulate);
+    if (narrow) {
+        constexpr int BNX = 56;
+        const size_t smem = STAGES * (OPK_BYTES + BK * (BNX * 16 + 32));
+        JDFT_CUDA(ensure_smem(k_gemm_expand<BNX, 4, 1>, smem));
+        dim3 grid((unsigned)((Nn + BNX - 1) / BNX), (unsigned)rt);
+        k_gemm_expand<BNX, 4, 1><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, accumulate);
+    } else {
+        const size_t smem = STAGES * (OPK_BYTES + OPN_BYTES);
+        JDFT_CUDA(ensure_smem(k_gemm_expand<BN, 2, 2>, smem));
+        dim3 grid((unsigned)((Nn + BN - 1) / BN), (unsigned)rt);
+        k_gemm_expand<BN, 2, 2><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, accumulate);
+    }
     jdft_prof_end(b, JDFT_K_GEMM_EXPAND, st);
     JDFT_LAUNCH_CHECK("k_gemm_expand");
     return JDFT_OK;

@@ -49,14 +49,16 @@ __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld
 }
 
 // ---------------------------------------------------------------------------------------------- dot-K GEMM
-template <bool CONJY, bool TRI>
+// BN_ = 64, or 48 when the column extent is a multiple of 48 but not of 64 (np = 288, 864: no zero-padded DMMAs)
+template <bool CONJY, bool TRI, int BN_>
 __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
                                                         const double2 *__restrict__ Y, const int Cn, const int64_t K,
                                                         const int ktiles_per_split, double2 *__restrict__ part) {
     extern __shared__ __align__(16) char smem[];
     char *sX = smem, *sY = smem + STAGES * OPK_BYTES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wr = (warp >> 1) * 32, wc = (warp & 1) * 32;
+    constexpr int NTL = BN_ / 16;   // 8-wide DMMA tiles per warp along the columns
+    const int wr = (warp >> 1) * 32, wc = (warp & 1) * (BN_ / 2);
     // tri: X == Y and the result is Hermitian; blockIdx.x enumerates the lower-triangle tiles (row tile >= col tile)
     int tr = blockIdx.y, tc = blockIdx.x;
     if constexpr (TRI) {
@@ -66,23 +68,24 @@ __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restric
         while (tr * (tr + 1) / 2 > t) tr--;
         tc = t - tr * (tr + 1) / 2;
     }
-    const int row0 = tr * BM, col0 = tc * BN;
+    const int row0 = tr * BM, col0 = tc * BN_;
+    const int cend = min(Cn, col0 + BN_);   // rows of Y this tile owns (the loader fills the rest of its 64 rows with zeros)
     const int64_t ktiles = (K + BK - 1) / BK;
     const int64_t kt0 = (int64_t)blockIdx.z * ktiles_per_split;
     int64_t kt1 = kt0 + ktiles_per_split;
     if (kt1 > ktiles) kt1 = ktiles;
     const int nkt = (int)(kt1 - kt0);
 
-    double cr[4][4][2], ci[4][4][2];
+    double cr[4][NTL][2], ci[4][NTL][2];
 #pragma unroll
     for (int i = 0; i < 4; i++)
 #pragma unroll
-        for (int j = 0; j < 4; j++) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+        for (int j = 0; j < NTL; j++) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
 
     for (int s = 0; s < STAGES - 1; s++) {
         if (s < nkt) {
             load_opk(sX + s * OPK_BYTES, X, K, Rn, row0, (kt0 + s) * BK, K, tid);
-            load_opk(sY + s * OPK_BYTES, Y, K, Cn, col0, (kt0 + s) * BK, K, tid);
+            load_opk(sY + s * OPK_BYTES, Y, K, cend, col0, (kt0 + s) * BK, K, tid);
         }
         cp_async_commit();
     }
@@ -95,24 +98,24 @@ __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restric
             if (nx < nkt) {
                 const int slot = nx % STAGES;
                 load_opk(sX + slot * OPK_BYTES, X, K, Rn, row0, (kt0 + nx) * BK, K, tid);
-                load_opk(sY + slot * OPK_BYTES, Y, K, Cn, col0, (kt0 + nx) * BK, K, tid);
+                load_opk(sY + slot * OPK_BYTES, Y, K, cend, col0, (kt0 + nx) * BK, K, tid);
             }
             cp_async_commit();
         }
         const char *bx = sX + (kt % STAGES) * OPK_BYTES, *by = sY + (kt % STAGES) * OPK_BYTES;
 #pragma unroll
         for (int kk = 0; kk < BK / 4; kk++) {
-            double2 a[4], bq[4];
+            double2 a[4], bq[NTL];
 #pragma unroll
             for (int i = 0; i < 4; i++)
                 a[i] = *reinterpret_cast<const double2 *>(bx + kk * KBLK_BYTES + (wr + 8 * i) * 64 + fo);
 #pragma unroll
-            for (int j = 0; j < 4; j++)
+            for (int j = 0; j < NTL; j++)
                 bq[j] = *reinterpret_cast<const double2 *>(by + kk * KBLK_BYTES + (wc + 8 * j) * 64 + fo);
 #pragma unroll
             for (int i = 0; i < 4; i++)
 #pragma unroll
-                for (int j = 0; j < 4; j++) {
+                for (int j = 0; j < NTL; j++) {
                     // X (Yr -/+ i Yi):  conj: Cr += XrYr + XiYi, Ci += XiYr - XrYi ; else Cr += XrYr - XiYi, Ci += XiYr + XrYi
                     const double yi = CONJY ? bq[j].y : -bq[j].y;
                     dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
@@ -129,7 +132,7 @@ __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restric
         const int r = row0 + wr + 8 * i + (lane >> 2);
         if (r >= Rn) continue;
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < NTL; j++) {
             const int c = col0 + wc + 8 * j + 2 * (lane & 3);
             if (c < Cn) P[(size_t)r * Cn + c] = make_double2(cr[i][j][0], ci[i][j][0]);
             if (c + 1 < Cn) P[(size_t)r * Cn + c + 1] = make_double2(cr[i][j][1], ci[i][j][1]);
@@ -276,7 +279,11 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     // X^+ X is Hermitian: compute the lower-triangle tiles only and mirror them in the reduction
     const int tri = (X == Y && Rn == Cn && conjY && !dscale && BM == BN) ? 1 : 0;
     const int trow = (Rn + BM - 1) / BM;
-    const int tiles = tri ? trow * (trow + 1) / 2 : trow * ((Cn + BN - 1) / BN);
+    // column tile: 48 instead of 64 when that removes a noticeable share of zero padding (np = 288: 320 -> 288 columns)
+    const int pad64 = ((Cn + 63) / 64) * 64, pad48 = ((Cn + 47) / 48) * 48;
+    const int bn = (!tri && Cn > 64 && pad48 * 100 < pad64 * 93) ? 48 : 64;  // measured: pays at 10 % padding (np = 288), not at 3.6 % (np = 864)
+    const int tcol = (Cn + bn - 1) / bn;
+    const int tiles = tri ? trow * (trow + 1) / 2 : trow * tcol;
     const size_t one = (size_t)Rn * Cn * 16;
     // Split K so that the grid fills whole waves of the 148 SMs x 2 resident CTAs (184 registers x 128 threads):
     // among 1..6 waves take the first whose fill tiles*nsplit / (waves*slots) reaches 93 %, else the best one.
@@ -302,18 +309,20 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     nsplit = (ktiles + per - 1) / per;
     if (nsplit < 1) nsplit = 1;
     const size_t smem = 2 * STAGES * OPK_BYTES;
-    dim3 grid(tri ? tiles : (Cn + BN - 1) / BN, tri ? 1 : trow, (unsigned)nsplit);
+    dim3 grid(tri ? tiles : tcol, tri ? 1 : trow, (unsigned)nsplit);
     jdft_prof_begin(b, JDFT_K_GEMM_DOTK, st);
-    if (tri) {
-        JDFT_CUDA(ensure_smem(k_gemm_dotk<true, true>, smem));
-        k_gemm_dotk<true, true><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
-    } else if (conjY) {
-        JDFT_CUDA(ensure_smem(k_gemm_dotk<true, false>, smem));
-        k_gemm_dotk<true, false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
-    } else {
-        JDFT_CUDA(ensure_smem(k_gemm_dotk<false, false>, smem));
-        k_gemm_dotk<false, false><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, (int)per, (double2 *)scratch);
-    }
+#define JDFT_DOTK_LAUNCH(CJ, TR, BNX)                                                                          \
+    do {                                                                                                        \
+        JDFT_CUDA(ensure_smem(k_gemm_dotk<CJ, TR, BNX>, smem));                                                 \
+        k_gemm_dotk<CJ, TR, BNX><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, \
+                                                               (int)per, (double2 *)scratch);                  \
+    } while (0)
+    if (tri) JDFT_DOTK_LAUNCH(true, true, 64);
+    else if (conjY && bn == 48) JDFT_DOTK_LAUNCH(true, false, 48);
+    else if (conjY) JDFT_DOTK_LAUNCH(true, false, 64);
+    else if (bn == 48) JDFT_DOTK_LAUNCH(false, false, 48);
+    else JDFT_DOTK_LAUNCH(false, false, 64);
+#undef JDFT_DOTK_LAUNCH
     jdft_prof_end(b, JDFT_K_GEMM_DOTK, st);
     JDFT_LAUNCH_CHECK("k_gemm_dotk");
     const int64_t total = (int64_t)Rn * Cn;

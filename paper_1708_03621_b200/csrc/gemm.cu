@@ -69,7 +69,8 @@ __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restric
         tc = t - tr * (tr + 1) / 2;
     }
     const int row0 = tr * BM, col0 = tc * BN_;
-    const int cend = min(Cn, col0 + BN_);   // rows of Y this tile owns (the loader fills the rest of its 64 rows with zeros)
+    // rows of Y this tile owns (the loader fills the rest of its 64 rows with zeros); 64: exactly the original code path
+    const int cend = BN_ == 64 ? Cn : min(Cn, col0 + BN_);
     const int64_t ktiles = (K + BK - 1) / BK;
     const int64_t kt0 = (int64_t)blockIdx.z * ktiles_per_split;
     int64_t kt1 = kt0 + ktiles_per_split;

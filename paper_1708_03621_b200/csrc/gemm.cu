@@ -287,7 +287,7 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     const int tiles = tri ? trow * (trow + 1) / 2 : trow * tcol;
     const size_t one = (size_t)Rn * Cn * 16;
     // Split K so that the grid fills whole waves of the 148 SMs x 2 resident CTAs (184 registers x 128 threads):
-    // among 1..6 waves take the first whose fill tiles*nsplit / (waves*slots) reaches 93 %, else the best one.
+    // among 1..6 waves take the smallest count whose fill tiles*nsplit / (waves*slots) is within 2 % of the best (stop at 97 %).
     const int64_t slots = 148 * 2;
     const int64_t max_by_k = ktiles / 16 > 0 ? ktiles / 16 : 1;              // at least 16 k-tiles (128 k) per slice
     const int64_t max_by_ws = (int64_t)(scratch_bytes / one);
@@ -302,8 +302,8 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
         const int64_t ctas = ns * tiles;
         const int64_t waves = (ctas + slots - 1) / slots;
         const double fill = (double)ctas / (double)(waves * slots);
-        if (fill > best + 1e-9) { best = fill; nsplit = ns; }
-        if (best >= 0.93) break;
+        if (fill > best + 0.02) { best = fill; nsplit = ns; }   // more waves (more partials) only for > 2 % better fill
+        if (best >= 0.97) break;
     }
     int64_t per = (ktiles + nsplit - 1) / nsplit;
     if (per < 1) per = 1;

@@ -393,10 +393,21 @@ def run_ours(args):
         ms_h = t_op(lambda: jd.jdft_pcm_hessian(gs, epsr, phi, hout))
         a_s, b_s = gs.ncol * S[2], gs.npl * S[1] * S[2]
         hess_bytes = 3 * nf * 16 * (4 * a_s + 4 * b_s + 2 * gs.nG) + nf * 16 * 8 * gs.nG + 8 * int(np.prod(S))
+        # stand-alone I and J (row a10) on 16 bands: the full real-space block is written / read once
+        nbI = min(nb, 16)
+        CI = k["C"][:nbI].contiguous()
+        psiI = torch.empty((nbI,) + tuple(S), dtype=torch.complex128, device="cuda")
+        CJ = torch.empty_like(CI)
+        ms_I = t_op(lambda: jd.jdft_apply_I(k["gb"], CI, psiI))
+        ms_J = t_op(lambda: jd.jdft_apply_J(k["gb"], psiI, CJ))
+        ij_bytes = nbI * 16 * (i["nG"] + 2 * i["a"] + 2 * i["b"] + i["N"])
+        extras_ij = {"apply_I": {"ms": ms_I, "bands": nbI, "alg_GB/s": ij_bytes / (ms_I * 1e-3) / 1e9},
+                     "apply_J": {"ms": ms_J, "bands": nbI, "alg_GB/s": ij_bytes / (ms_J * 1e-3) / 1e9}}
         extras = {"pcm_hessian": {"ms": ms_h, "fields": nf, "nG": gs.nG, "fields_per_s": nf / (ms_h * 1e-3),
                                   "alg_GB/s": hess_bytes / (ms_h * 1e-3) / 1e9},
                   "density": {"ms": ms_d, "bands_per_s": nb / (ms_d * 1e-3), "alg_GB/s": dens_bytes / (ms_d * 1e-3) / 1e9},
                   "subspace": {"ms": ms_s, "TFLOP/s": 8.0 * nb * nb * i["nG"] / (ms_s * 1e-3) / 1e12}}
+        extras.update(extras_ij)
 
     if rank != 0:
         return

@@ -77,6 +77,16 @@ def test_null_and_bad_arguments_return_status_codes_without_a_device(lib):
     lib.jdft_basis_create.argtypes = [vp, vp, ctypes.c_double, vp, ctypes.c_int, ctypes.POINTER(vp)]
     h = vp()
     assert lib.jdft_basis_create(None, None, 1.0, None, 0, ctypes.byref(h)) == EINVAL
+    # the calls added for SURVEY 8(f) validate the same way
+    lib.jdft_subspace.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp]
+    assert lib.jdft_subspace(None, None, 1, None, 1, None, None) == EINVAL
+    lib.jdft_density.argtypes = [vp, vp, ctypes.c_int, vp, vp, ctypes.c_int, vp]
+    assert lib.jdft_density(None, None, 1, None, None, 0, None) == EINVAL
+    for fn in (lib.jdft_gradient, lib.jdft_divergence):
+        fn.argtypes = [vp, vp, ctypes.c_int, vp, vp]
+        assert fn(None, None, 1, None, None) == EINVAL
+    lib.jdft_pcm_hessian.argtypes = [vp, vp, vp, ctypes.c_int, vp, vp]
+    assert lib.jdft_pcm_hessian(None, None, None, 1, None, None) == EINVAL
     lib.jdft_version.restype = ctypes.c_char_p
     assert lib.jdft_version().startswith(b"jdft-b200")
 

@@ -607,6 +607,75 @@ __global__ void __launch_bounds__(Hyb<LT>::NT) k_rows_hyb(const double2 *__restr
     }
 }
 
+// Last pass of I (MODE 1: occupied planes of W2 -> full real-space block) and first pass of I^+ / J (MODE 2: the
+// reverse), same hybrid as k_rows_hyb: pencil pairs with 256-bit loads in the first pass, single pencils in the last.
+template <int LT, int MODE>
+__global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_io_hyb(const double2 *__restrict__ tw, const int S1, const int S2,
+                                                               const int npl, const int *__restrict__ planeof,
+                                                               double2 *__restrict__ W2, double2 *__restrict__ psi) {
+    using C = Tuned<LT>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, H = T / 2, NT = Hyb<LT>::NT, L = LT;
+    constexpr int SIGN = MODE == 1 ? +1 : -1;
+    extern __shared__ double2 smem[];
+    double2 *A = smem;
+    __shared__ int s_planeof[L];
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y, b = blockIdx.z;
+    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    __syncthreads();
+    const size_t plane = (size_t)S1 * S2;
+    double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
+    double2 *pb = psi + (size_t)b * L * plane + (size_t)i1 * S2 + t0;
+    const int tmax = S2 - t0;  // even
+    if (tid < R2 * H) {
+        const int l = tid % H, bf = tid / H;
+        double2 a0[R1], a1[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) {
+            const int row = bf + k * R2;
+            a0[k] = a1[k] = make_double2(0.0, 0.0);
+            if (MODE == 1) {
+                const int p = s_planeof[row];
+                if (p >= 0 && 2 * l < tmax) ld256(W2b + p * plane + 2 * l, a0[k], a1[k]);
+            } else {
+                if (2 * l < tmax) ld256(pb + row * plane + 2 * l, a0[k], a1[k]);
+            }
+        }
+        Dft<R1, SIGN>::run(a0);
+        Dft<R1, SIGN>::run(a1);
+#pragma unroll
+        for (int j = 1; j < R1; j++) {
+            double2 wv = __ldg(tw + bf * j);
+            if (SIGN < 0) wv.y = -wv.y;
+            a0[j] = cmul(a0[j], wv);
+            a1[j] = cmul(a1[j], wv);
+        }
+#pragma unroll
+        for (int j = 0; j < R1; j++) {
+            A[(bf * R1 + j) * T + l] = a0[j];
+            A[(bf * R1 + j) * T + H + l] = a1[j];
+        }
+    }
+    __syncthreads();
+    if (tid < R1 * T) {
+        const int x = tid % T, bf = tid / T;
+        const int t = x < H ? 2 * x : 2 * (x - H) + 1;
+        double2 a[R2];
+#pragma unroll
+        for (int k = 0; k < R2; k++) a[k] = A[(bf + k * R1) * T + x];
+        Dft<R2, SIGN>::run(a);
+#pragma unroll
+        for (int j = 0; j < R2; j++) {
+            const int row = bf + R1 * j;
+            if (MODE == 1) {
+                if (t < tmax) pb[row * plane + t] = a[j];
+            } else {
+                const int p = s_planeof[row];
+                if (p >= 0 && t < tmax) W2b[p * plane + t] = a[j];
+            }
+        }
+    }
+}
+
 // Density, tuned: last pass of I for the two-pass lengths with the |psi|^2 accumulators in REGISTERS.  A CTA owns the
 // tile (i1, 16 adjacent i2) and walks the bands of the batch in order; in the last pass (radix R2, one round) a
 // thread always produces the same rows bf + R1 j of the same pencil, so it keeps their R2 partial sums itself.
@@ -816,6 +885,9 @@ __global__ void k_diag(const int64_t nG, const int64_t total, const double f0, c
 }
 
 // ------------------------------------------------------------------------------------------------ launch helpers
+// the 256-bit global accesses of the pair / hybrid kernels need 32-byte aligned arrays (the ABI only asks for 16)
+inline bool aligned32(const void *a, const void *b = nullptr) { return ((((uintptr_t)a) | ((uintptr_t)b)) & 31) == 0; }
+
 template <class K>
 cudaError_t ensure_smem(K kernel, size_t bytes) {
     if (bytes <= 40 * 1024) return cudaSuccess;  // static __shared__ tables count against the 48 KB default too
@@ -908,7 +980,7 @@ int launch_rows(const jdft_basis *b, int nbt, double2 *W1, double2 *W2, cudaStre
     jdft_prof_begin(b, FWD ? JDFT_K_ROWS_FWD : JDFT_K_ROWS_INV, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         if constexpr (LT == 128) {  // measured: 1.07 -> 0.94 ms at 128 (91 % of the HBM roofline), slower at 80
-            if (b->S[2] % 2 == 0 && b->opt_pair) {
+            if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(W1, W2)) {
                 using C = Tuned<LT>;
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
                 JDFT_CUDA(ensure_smem(k_rows_hyb<LT, FWD>, sm2));
@@ -943,7 +1015,7 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
     jdft_prof_begin(b, JDFT_K_PLANES, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         if constexpr (MODE == 0 && Pair<LT>::ok && LT == 72) {  // measured: +7 % at 72 (32 pencils/CTA), -12 % at 80 (16 pencils, 80 threads)
-            if (b->S[2] % 2 == 0 && b->opt_pair) {
+            if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(W2) && (((uintptr_t)V) & 15) == 0) {
                 using Q = Pair<LT>;
                 const size_t sm2 = (size_t)Q::G * L * Q::T * sizeof(double2);
                 JDFT_CUDA(ensure_smem(k_planes_fused2<LT>, sm2));
@@ -954,8 +1026,20 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
                 return JDFT_OK;
             }
         }
+        if constexpr (MODE != 0 && (LT == 128 || LT == 80)) {
+            if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(W2, psi)) {
+                using C = Tuned<LT>;
+                const size_t sm2 = (size_t)L * C::T * sizeof(double2);
+                JDFT_CUDA(ensure_smem(k_planes_io_hyb<LT, MODE>, sm2));
+                dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
+                k_planes_io_hyb<LT, MODE><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, psi);
+                jdft_prof_end(b, JDFT_K_PLANES, st);
+                JDFT_LAUNCH_CHECK("k_planes_io_hyb");
+                return JDFT_OK;
+            }
+        }
         if constexpr (MODE == 0 && (LT == 128 || LT == 80)) {  // 72 runs the full pair kernel above (hybrid measured slower)
-            if (b->S[2] % 2 == 0 && b->opt_pair) {
+            if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(W2)) {
                 using C = Tuned<LT>;
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
                 JDFT_CUDA(ensure_smem(k_planes_fused_h<LT>, sm2));

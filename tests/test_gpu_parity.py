@@ -426,3 +426,11 @@ def test_planes_pair_kernel_matches(ref, jd, cfg_id):
     b = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
     assert rel_err_per_band(a, want) <= TOL and rel_err_per_band(b, want) <= TOL
     assert rel_err_per_band(a, b) <= 1e-13
+    # a workspace that is only 16-byte aligned (all the ABI requires): the 256-bit kernels must step aside
+    jd.jdft_set_option(c.gb, "planes_pair", 1)
+    ws = torch.empty(jd.jdft_workspace_bytes(c.gb, c.nb, max(c.nb, c.P.shape[0])) + 64, dtype=torch.uint8, device="cuda")
+    jd.jdft_set_workspace(c.gb, ws[16:])
+    d = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+    assert rel_err_per_band(d, want) <= TOL
+    psi = jd.jdft_apply_I(c.gb, dev(c.C))
+    assert rel_err_per_band(jd.jdft_apply_J(c.gb, psi).cpu().numpy(), c.C) <= 1e-13

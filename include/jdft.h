@@ -27,7 +27,8 @@
  *   Vnl         = P D P^+ with P = [np][nG] (projector-major) and D given as data
  *
  * Pointers.  Unless marked HOST, every data pointer is a DEVICE pointer on the basis' device, owned by
- * the caller (e.g. a torch tensor's data_ptr()), 16-byte aligned.  The library owns only the basis
+ * the caller (e.g. a torch tensor's data_ptr()), 16-byte aligned (32-byte aligned arrays and workspace, as any
+ * allocator gives, let the library pick its 256-bit load/store kernels; results are the same either way).  The library owns only the basis
  * object.  The hot path allocates nothing and never synchronises with the host: all scratch comes from
  * the caller-supplied workspace, and kernels are enqueued on the caller's stream.  Input and output
  * arrays must not alias unless stated.

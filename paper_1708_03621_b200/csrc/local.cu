@@ -676,6 +676,75 @@ __global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_io_hyb(const double2 *__
     }
 }
 
+// Density with the hybrid first pass (pencil pairs, 256-bit loads) of k_planes_io_hyb and register accumulators.
+template <int LT>
+__global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_density_hyb(const double2 *__restrict__ tw, const int S1, const int S2,
+                                                                    const int npl, const int *__restrict__ planeof,
+                                                                    const double2 *__restrict__ W2, const double *__restrict__ f,
+                                                                    const int nbt, double *__restrict__ n, const int accumulate) {
+    using C = Tuned<LT>;
+    constexpr int R1 = C::R1, R2 = C::R2, T = C::T, H = T / 2, NT = Hyb<LT>::NT, L = LT;
+    extern __shared__ double2 smem[];
+    double2 *A = smem;
+    __shared__ int s_planeof[L];
+    const int tid = threadIdx.x, t0 = blockIdx.x * T, i1 = blockIdx.y;
+    for (int i = tid; i < L; i += NT) s_planeof[i] = planeof[i];
+    __syncthreads();
+    const size_t plane = (size_t)S1 * S2;
+    const int tmax = S2 - t0;  // even
+    const int x = tid % T, bfl = tid / T;
+    const int tl = x < H ? 2 * x : 2 * (x - H) + 1;
+    const bool act = tid < R1 * T;
+    double acc[R2];
+#pragma unroll
+    for (int j = 0; j < R2; j++) acc[j] = 0.0;
+    for (int b = 0; b < nbt; b++) {
+        const double2 *W2b = W2 + (size_t)b * npl * plane + (size_t)i1 * S2 + t0;
+        if (tid < R2 * H) {
+            const int l = tid % H, bf = tid / H;
+            double2 a0[R1], a1[R1];
+#pragma unroll
+            for (int k = 0; k < R1; k++) {
+                const int p = s_planeof[bf + k * R2];
+                a0[k] = a1[k] = make_double2(0.0, 0.0);
+                if (p >= 0 && 2 * l < tmax) ld256(W2b + p * plane + 2 * l, a0[k], a1[k]);
+            }
+            Dft<R1, +1>::run(a0);
+            Dft<R1, +1>::run(a1);
+#pragma unroll
+            for (int j = 1; j < R1; j++) {
+                const double2 wv = __ldg(tw + bf * j);
+                a0[j] = cmul(a0[j], wv);
+                a1[j] = cmul(a1[j], wv);
+            }
+#pragma unroll
+            for (int j = 0; j < R1; j++) {
+                A[(bf * R1 + j) * T + l] = a0[j];
+                A[(bf * R1 + j) * T + H + l] = a1[j];
+            }
+        }
+        __syncthreads();
+        if (act) {
+            const double fb = f[b];
+            double2 a[R2];
+#pragma unroll
+            for (int k = 0; k < R2; k++) a[k] = A[(bfl + k * R1) * T + x];
+            Dft<R2, +1>::run(a);
+#pragma unroll
+            for (int j = 0; j < R2; j++) acc[j] = fma(fb, a[j].x * a[j].x + a[j].y * a[j].y, acc[j]);
+        }
+        __syncthreads();
+    }
+    if (act && tl < tmax) {
+        double *o = n + (size_t)i1 * S2 + t0 + tl;
+#pragma unroll
+        for (int j = 0; j < R2; j++) {
+            double *q = o + (size_t)(bfl + R1 * j) * plane;
+            *q = accumulate ? *q + acc[j] : acc[j];
+        }
+    }
+}
+
 // Density, tuned: last pass of I for the two-pass lengths with the |psi|^2 accumulators in REGISTERS.  A CTA owns the
 // tile (i1, 16 adjacent i2) and walks the bands of the batch in order; in the last pass (radix R2, one round) a
 // thread always produces the same rows bf + R1 j of the same pencil, so it keeps their R2 partial sums itself.
@@ -1170,7 +1239,20 @@ extern "C" int jdft_density(const jdft_basis *b, const double *C_, int nb, const
         const int acc = (accumulate || b0 > 0) ? 1 : 0;
         jdft_prof_begin(b, JDFT_K_PLANES, st);
         SPEC_SWITCH(L, b->opt_force_generic, {
-            if constexpr (Tuned<LT>::ok) {
+            bool hyb = false;
+            if constexpr (LT == 128) {  // measured: 3.20 -> 2.73 ms on config 3; slower at 80
+                if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(w.W2)) {
+                    using C = Tuned<LT>;
+                    const size_t sm2 = (size_t)L * C::T * sizeof(double2);
+                    JDFT_CUDA(ensure_smem(k_planes_density_hyb<LT>, sm2));
+                    dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1]);
+                    k_planes_density_hyb<LT><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
+                                                                      f + b0, nbt, n, acc);
+                    hyb = true;
+                }
+            }
+            if (hyb) {
+            } else if constexpr (Tuned<LT>::ok) {
                 using C = Tuned<LT>;
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
                 JDFT_CUDA(ensure_smem(k_planes_density_tuned<LT>, sm2));

@@ -26,15 +26,18 @@ struct Cfg {
     static constexpr int TP = T + 1;
     // resident CTAs per SM the register allocation is bounded for (latency-bound kernels: more warps in flight win)
     static constexpr int RMAX = R0 > R1 ? (R0 > R2 ? R0 : R2) : (R1 > R2 ? R1 : R2);
-    static constexpr int FIT = ok ? 65536 / (T * (LT / R0) * (RMAX >= 15 ? 80 : (RMAX >= 12 ? 72 : 40))) : 1;
+    static constexpr int FIT = ok ? 65536 / (T * (LT / R0) / ((NP == 2 && LT / R0 == 2 * (LT / RL)) ? 2 : 1) * (RMAX >= 15 ? 80 : (RMAX >= 12 ? 72 : 40))) : 1;
     static constexpr int MINB_DEF = FIT < 1 ? 1 : (FIT > 6 ? 6 : FIT);
     // measured choices for the lengths of the five workloads (profiles/), the rule for the rest
-    static constexpr int MINB_INV = LT == 216 ? 5 : (LT == 128 ? 4 : MINB_DEF), MINB_FWD = (LT == 216 || LT == 128) ? 4 : MINB_DEF;
+    static constexpr int MINB_INV = LT == 216 ? 5 : (LT == 128 ? 6 : MINB_DEF), MINB_FWD = LT == 216 ? 4 : (LT == 128 ? 6 : MINB_DEF);
     static constexpr int NBL = ok ? LT / RL : 1;                // butterflies per pencil in the last pass
     static constexpr int NB0 = ok ? LT / R0 : 1;                // ... in the first pass
     // ONE swizzled tile [L][T]; the shared -> shared passes run in a single round (threads = their work items) and
     // in place: every thread reads its butterfly, barrier, writes it back
-    static constexpr int NT = T * NB0;
+    // first pass in ROUNDS0 rounds: 2 when it has twice the butterflies of the last pass (128 = 8 x 16), so that no
+    // thread idles in the (heavier) last pass; both rounds are read before the barrier of the in-place update
+    static constexpr int ROUNDS0 = (NP == 2 && NB0 == 2 * NBL) ? 2 : 1;
+    static constexpr int NT = T * NB0 / ROUNDS0;
     static constexpr int NB1 = ok ? LT / R1 : 1;                // butterflies per pencil in the middle pass (3-pass plans)
     static_assert(NP != 3 || NB1 * T == NT, "middle pass must be exactly one round");
     static constexpr size_t smem = (size_t)LT * T * sizeof(double2);
@@ -115,24 +118,35 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tun
             X[F::sw(row, t)] = Cb[n];
         }
         __syncthreads();
-        // pass 0 (radix R0, s = 1), one round, in place: rows bf + k NB0 (zero outside the run) -> rows bf R0 + j
+        // pass 0 (radix R0, s = 1), in place: rows bf + k NB0 (zero outside the run) -> rows bf R0 + j; every round is
+        // read before the barrier, written after it
         {
-            const int t = tid % T, bf = tid / T;
-            const int m2w = s_m2w[t], len = t < nc ? s_n0[t + 1] - s_n0[t] : 0;
-            double2 a[R0];
+            constexpr int RD = F::ROUNDS0;
+            double2 a[RD][R0];
 #pragma unroll
-            for (int k = 0; k < R0; k++) {
-                const int row = bf + k * NB0;
-                int off = row - m2w;
-                if (off < 0) off += L;
-                a[k] = make_double2(0.0, 0.0);
-                if (off < len) a[k] = X[F::sw(row, t)];
+            for (int r = 0; r < RD; r++) {
+                const int w = tid + r * NT;
+                const int t = w % T, bf = w / T;
+                const int m2w = s_m2w[t], len = t < nc ? s_n0[t + 1] - s_n0[t] : 0;
+#pragma unroll
+                for (int k = 0; k < R0; k++) {
+                    const int row = bf + k * NB0;
+                    int off = row - m2w;
+                    if (off < 0) off += L;
+                    a[r][k] = make_double2(0.0, 0.0);
+                    if (off < len) a[r][k] = X[F::sw(row, t)];
+                }
             }
             __syncthreads();
-            Dft<R0, +1>::run(a);
-            tw_mul<R0, +1>(a, tw, bf);
 #pragma unroll
-            for (int j = 0; j < R0; j++) X[F::sw(bf * R0 + j, t)] = a[j];
+            for (int r = 0; r < RD; r++) {
+                const int w = tid + r * NT;
+                const int t = w % T, bf = w / T;
+                Dft<R0, +1>::run(a[r]);
+                tw_mul<R0, +1>(a[r], tw, bf);
+#pragma unroll
+                for (int j = 0; j < R0; j++) X[F::sw(bf * R0 + j, t)] = a[r][j];
+            }
         }
         __syncthreads();
         if constexpr (F::NP == 3) mid_pass_inplace<LT, +1>(X, tw);

@@ -413,7 +413,7 @@ def test_ultrasoft_overlap_and_dense_D_by_composition(case, jd):
     assert np.max(np.abs(M_gpu - M_def)) <= 1e-10 * np.max(np.abs(M_def))
 
 
-@pytest.mark.parametrize("cfg_id", [210, 211, 212, 213, 214, 215])
+@pytest.mark.parametrize("cfg_id", [210, 211, 212, 213, 214, 215, 216])
 def test_planes_pair_kernel_matches(ref, jd, cfg_id):
     """Plane length 72 runs K3 with two pencils per thread (256-bit global accesses); same result as the one-pencil
     kernel and as the oracle; lengths 128 and 80 run the hybrid (pairs in the first and last pass only; also K2/K4 at row

@@ -45,6 +45,7 @@ def _rot(name, S, cfg_id):
 _LEN_BOXES = [(48, 96, 100), (96, 100, 48), (100, 48, 96), (120, 144, 160), (144, 160, 120), (160, 120, 144),
               (192, 256, 32), (256, 32, 192), (32, 192, 256)]
 TEST_CONFIGS[210] = _rot("t_len_72x40x48", (72, 40, 48), 210)   # plane length 72: the two-pencils-per-thread K3
+TEST_CONFIGS[216] = _rot("t_len_24x32x128", (24, 32, 128), 216)  # column length 128: two-round first pass in K1
 TEST_CONFIGS[214] = _rot("t_len_128x80x27", (128, 80, 27), 214)  # odd S2: the pair / hybrid kernels must step aside
 TEST_CONFIGS[215] = _rot("t_len_72x128x25", (72, 128, 25), 215)
 TEST_CONFIGS[213] = _rot("t_len_24x128x32", (24, 128, 32), 213)  # row length 128: hybrid pair/single K2, K4

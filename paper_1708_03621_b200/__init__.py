@@ -12,7 +12,7 @@ import importlib
 def __getattr__(name):
     if name.startswith("__"):
         raise AttributeError(name)
-    if name in ("build", "binding"):  # submodules: `from paper_1708_03621_b200 import build` must not load the .so
+    if name in ("build", "binding", "sharding"):  # submodules: `from paper_1708_03621_b200 import build` must not load the .so
         return importlib.import_module(__name__ + "." + name)
     binding = importlib.import_module(__name__ + ".binding")
     try:

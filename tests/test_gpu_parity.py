@@ -434,3 +434,43 @@ def test_planes_pair_kernel_matches(ref, jd, cfg_id):
     assert rel_err_per_band(d, want) <= TOL
     psi = jd.jdft_apply_I(c.gb, dev(c.C))
     assert rel_err_per_band(jd.jdft_apply_J(c.gb, psi).cpu().numpy(), c.C) <= 1e-13
+
+
+# ------------------------------------------------------------------------------------------ 8(f) rank 4: band shards
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("world", [1, 2, 3])
+def test_band_shards_compose_on_one_gpu(case, jd, world):
+    """The local operations each rank of sharding.py issues (one rank after the other on this one GPU, nothing waits
+    on anything): per-shard apply_H rows, the ring schedule's row-shard x column-shard overlap blocks, per-shard
+    density partial sums -- assembled, they equal the oracle on the unsharded arrays.  world = 1 goes through
+    sharding.py itself (no process group)."""
+    from paper_1708_03621_b200 import sharding as sh
+    rng = np.random.default_rng(91)
+    nb = case.nb
+    X = case.C + 0.1 * (rng.standard_normal(case.C.shape) + 1j * rng.standard_normal(case.C.shape))
+    f = rng.uniform(0.0, 2.0, nb)
+    Cd, Xd, fd = dev(case.C), dev(X), dev(f)
+    want_M, want_n = case.rb.overlap(case.C, X), case.rb.density(case.C, f)
+    want_H = case.rb.apply_H(case.V, case.P, case.D, case.C)
+    if world == 1:
+        M = sh.sharded_overlap(case.gb, Cd, Xd, nb).cpu().numpy()
+        n = sh.sharded_density(case.gb, Cd, fd).cpu().numpy()
+        HC = sh.sharded_apply_H(case.gb, dev(case.V), dev(case.P), dev(case.D), Cd).cpu().numpy()
+    else:
+        ranges = [sh.shard_range(nb, world, r) for r in range(world)]
+        M = np.zeros((nb, nb), dtype=np.complex128)
+        n = torch.zeros(case.rb.shape, dtype=torch.float64, device="cuda")
+        HC = np.zeros_like(case.C)
+        for lo, hi in ranges:                       # "rank" owning bands lo:hi
+            if hi == lo:
+                continue
+            for r0, r1 in ranges:                   # the row shard that is resident at this ring step
+                if r1 > r0:
+                    M[r0:r1, lo:hi] = jd.jdft_overlap(case.gb, Cd[r0:r1].contiguous(), Xd[lo:hi].contiguous()).cpu().numpy()
+            n += jd.jdft_density(case.gb, Cd[lo:hi].contiguous(), fd[lo:hi].contiguous())   # the all-reduce's sum
+            HC[lo:hi] = jd.jdft_apply_H(case.gb, dev(case.V), dev(case.P), dev(case.D), Cd[lo:hi].contiguous()).cpu().numpy()
+        n = n.cpu().numpy()
+    assert rel_err_per_band(M.T, want_M.T) <= TOL
+    assert np.linalg.norm(n - want_n) <= TOL * np.linalg.norm(want_n)
+    assert rel_err_per_band(HC, want_H) <= TOL

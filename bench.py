@@ -486,7 +486,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", action="store_true", help="also time jdft_density and jdft_subspace (SURVEY 8(f) rank 1)")
     ap.add_argument("--overlap", action="store_true",
-                    help="run the projection GEMM on a side stream beside the FFT pipeline (measured +1-2 %; off by default)")
+                    help="run the projection GEMM on a side stream beside the FFT pipeline (measured +1-2 %%; off by default)")
     args = ap.parse_args()
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) == 0:

@@ -78,3 +78,8 @@ def test_algorithmic_bytes_match_design_formula():
     assert tot == want
     assert bench.algorithmic(info, "gemm_dotk", 1) == 8 * 128 * 256 * 23928
     assert bench.algorithmic(info, "gemm_expand", 1) == 8 * 128 * 256 * 23928
+
+
+def test_bench_help_renders():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--help"], capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0 and "--config" in out.stdout

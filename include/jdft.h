@@ -87,6 +87,8 @@ int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
  * tests), "overlap_gemm" (0/1, default 0: apply_H forks B = D P^+ C onto a basis-owned side stream beside the FFT
  * pipeline and joins before HC += P B; uses basis-owned events, so not for concurrent calls on one basis),
  * "planes_pair" (0/1, default 1: K3 with two pencils per thread where that variant exists),
+ * "planes_prune" (0/1, default 1: K3 hybrid with radix-8 butterflies pruned to the sphere's extent along axis 0
+ * when planes [L/4, 3L/4) are empty),
  * "profile_kernel" (see diagnostics)                                                                    */
 int jdft_set_option(jdft_basis *b, const char *key, int64_t value);
 

@@ -46,6 +46,7 @@ struct jdft_basis {
     // runs on the caller's stream
     int64_t opt_overlap;
     int64_t opt_pair;                         // K3 with two pencils per thread where available ("planes_pair")
+    int64_t opt_prune;                        // K3 hybrid: radix-8 butterflies pruned to the occupied planes ("planes_prune")
     cudaStream_t side;
     cudaEvent_t ev_fork, ev_join;
     // optional per-kernel event timing (option "profile_kernel" = one of JDFT_K_*; 0 = off).  Diagnostics only.

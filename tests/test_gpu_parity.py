@@ -474,3 +474,22 @@ def test_band_shards_compose_on_one_gpu(case, jd, world):
     assert rel_err_per_band(M.T, want_M.T) <= TOL
     assert np.linalg.norm(n - want_n) <= TOL * np.linalg.norm(want_n)
     assert rel_err_per_band(HC, want_H) <= TOL
+
+
+@pytest.mark.parametrize("cfg_id", [211, 212, 217])
+def test_planes_pruned_butterflies_match(ref, jd, cfg_id):
+    """K3 hybrid (plane lengths 80, 128): radix-8 first/last butterflies pruned to the sphere's axis-0 extent (inputs /
+    outputs 2..5 are empty planes).  211 (|m0| <= 13 of 80) and 212 (|m0| <= 21 of 128) take the pruned kernel, 217
+    (|m0| <= 22 of 80, planes 20..22 occupied) must fall back; all equal the unpruned kernel and the oracle."""
+    c = Case(ref, jd, cfg_id)
+    m0 = c.rb.iG[:, 0]
+    L, R2 = c.rb.shape[0], c.rb.shape[0] // 8
+    assert (max(m0.max(), -m0.min()) < 2 * R2) == (cfg_id != 217)
+    want = c.rb.apply_H(c.V, c.P, c.D, c.C)
+    args = (dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C))
+    a = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+    jd.jdft_set_option(c.gb, "planes_prune", 0)
+    b = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+    jd.jdft_set_option(c.gb, "planes_prune", 1)
+    assert rel_err_per_band(a, want) <= TOL and rel_err_per_band(b, want) <= TOL
+    assert rel_err_per_band(a, b) <= 1e-13

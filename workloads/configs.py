@@ -51,6 +51,8 @@ TEST_CONFIGS[215] = _rot("t_len_72x128x25", (72, 128, 25), 215)
 TEST_CONFIGS[213] = _rot("t_len_24x128x32", (24, 128, 32), 213)  # row length 128: hybrid pair/single K2, K4
 TEST_CONFIGS[212] = _rot("t_len_128x24x32", (128, 24, 32), 212)  # plane length 128: hybrid pair/single K3
 TEST_CONFIGS[211] = _rot("t_len_80x27x32", (80, 27, 32), 211)   # plane length 80: two tiles per CTA, odd S1 (idle group)
+# plane length 80 with |m0| up to 22 >= 2 R2 = 20: K3's pruned radix-8 butterflies must step aside
+TEST_CONFIGS[217] = dict(_rot("t_len_80x27x32_wide", (80, 27, 32), 217), Ecut=25.0)
 for _i, _S in enumerate(_LEN_BOXES):
     TEST_CONFIGS[201 + _i] = _rot("t_len_%dx%dx%d" % _S, _S, 201 + _i)
 

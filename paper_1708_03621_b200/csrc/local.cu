@@ -324,6 +324,34 @@ __global__ void __launch_bounds__(Tuned<LT>::NT, PlanesMinB<LT>::v) k_planes_fus
 // which cuts the load/store instruction count per pencil by ~30 % on the pipe that bounds k_planes_fused.
 // Shared tile [L][T] with the even pencils in the first half of a row and the odd ones in the second, so both
 // 16-byte accesses of a thread are lane-contiguous.  Requires S2 even (32-byte alignment of a pencil pair).
+// Radix-8 butterflies pruned to the sphere's extent along axis 0 (PR = true, R1 = 8): when the planes
+// [2 R2, 6 R2) hold no sphere point (|m0| < 2 R2, true for every workload of BASELINE.json at 80 and 128), inputs
+// 2..5 of every first-pass butterfly are zero and outputs 2..5 of every last-pass butterfly are discarded.
+// dft8_in0167: a[n] <- a0 + a1 w^n + a6 w^6n + a7 w^7n, w = exp(SIGN 2 pi i / 8)  (a[2..5] ignored on entry)
+template <int SIGN>
+__device__ __forceinline__ void dft8_in0167(double2 (&a)[8]) {
+    const double2 j6 = mul_i<SIGN>(a[6]);
+    const double2 e0 = cadd(a[0], a[6]), e2 = csub(a[0], a[6]), e1 = csub(a[0], j6), e3 = cadd(a[0], j6);
+    const double2 u = mul_w<SIGN, 1, 8>(a[1]), v = mul_w<SIGN, 7, 8>(a[7]);
+    const double2 o0 = cadd(a[1], a[7]), o2 = mul_i<SIGN>(csub(a[1], a[7]));
+    const double2 o1 = cadd(u, v), o3 = mul_i<SIGN>(csub(u, v));
+    a[0] = cadd(e0, o0); a[4] = csub(e0, o0);
+    a[1] = cadd(e1, o1); a[5] = csub(e1, o1);
+    a[2] = cadd(e2, o2); a[6] = csub(e2, o2);
+    a[3] = cadd(e3, o3); a[7] = csub(e3, o3);
+}
+// dft8_out0167: outputs 0, 1, 6, 7 of the full length-8 DFT (a[2..5] undefined on exit)
+template <int SIGN>
+__device__ __forceinline__ void dft8_out0167(double2 (&a)[8]) {
+    const double2 s0 = cadd(a[0], a[4]), s1 = cadd(a[1], a[5]), s2 = cadd(a[2], a[6]), s3 = cadd(a[3], a[7]);
+    const double2 d0 = csub(a[0], a[4]), d1 = csub(a[1], a[5]), d2 = csub(a[2], a[6]), d3 = csub(a[3], a[7]);
+    const double2 j2 = mul_i<SIGN>(d2), j3 = mul_i<SIGN>(d3);
+    a[0] = cadd(cadd(s0, s2), cadd(s1, s3));
+    a[6] = csub(csub(s0, s2), mul_i<SIGN>(csub(s1, s3)));
+    a[1] = cadd(cadd(d0, j2), mul_w<SIGN, 1, 8>(cadd(d1, j3)));
+    a[7] = cadd(csub(d0, j2), mul_w<SIGN, 7, 8>(csub(d1, j3)));
+}
+
 template <int LT>
 struct Pair {
     static constexpr int T = LT == 72 ? 32 : 16;       // pencils per CTA
@@ -339,7 +367,7 @@ __device__ __forceinline__ void ld256(const double2 *p, double2 &a, double2 &b) 
 __device__ __forceinline__ void st256(double2 *p, const double2 a, const double2 b) {
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
 }
-template <int LT>
+template <int LT, bool PR = false>
 __global__ void __launch_bounds__(Pair<LT>::NT) k_planes_fused2(const double2 *__restrict__ tw, const int S1, const int S2,
                                                                 const int npl, const int *__restrict__ planeof,
                                                                 double2 *__restrict__ W2, const double *__restrict__ V) {
@@ -364,12 +392,18 @@ __global__ void __launch_bounds__(Pair<LT>::NT) k_planes_fused2(const double2 *_
         double2 a0[R1], a1[R1];
 #pragma unroll
         for (int k = 0; k < R1; k++) {
+            if (PR && k >= 2 && k < 6) continue;
             const int p = s_planeof[bf + k * R2];
             a0[k] = a1[k] = make_double2(0.0, 0.0);
             if (p >= 0 && 2 * l < tmax) ld256(W2b + p * plane + 2 * l, a0[k], a1[k]);
         }
-        Dft<R1, +1>::run(a0);
-        Dft<R1, +1>::run(a1);
+        if constexpr (PR) {
+            dft8_in0167<+1>(a0);
+            dft8_in0167<+1>(a1);
+        } else {
+            Dft<R1, +1>::run(a0);
+            Dft<R1, +1>::run(a1);
+        }
 #pragma unroll
         for (int j = 1; j < R1; j++) {
             const double2 wv = __ldg(tw + bf * j);
@@ -432,10 +466,16 @@ __global__ void __launch_bounds__(Pair<LT>::NT) k_planes_fused2(const double2 *_
             a0[k] = A[(bf + k * R2) * T + l];
             a1[k] = A[(bf + k * R2) * T + H + l];
         }
-        Dft<R1, -1>::run(a0);
-        Dft<R1, -1>::run(a1);
+        if constexpr (PR) {
+            dft8_out0167<-1>(a0);
+            dft8_out0167<-1>(a1);
+        } else {
+            Dft<R1, -1>::run(a0);
+            Dft<R1, -1>::run(a1);
+        }
 #pragma unroll
         for (int j = 0; j < R1; j++) {
+            if (PR && j >= 2 && j < 6) continue;
             const int p = s_planeof[bf + R2 * j];
             if (p >= 0 && 2 * l < tmax) st256(W2b + p * plane + 2 * l, a0[j], a1[j]);
         }
@@ -453,36 +493,8 @@ struct Hyb {  // threads = the larger of the pair passes' and the middle pass' w
     static constexpr int NT = PAIRS > MID ? PAIRS : MID;
     static constexpr int MINB = LT == 128 ? 4 : 5;   // measured
 };
-// Radix-8 butterflies pruned to the sphere's extent along axis 0 (PR = true, R1 = 8): when the planes
-// [2 R2, 6 R2) hold no sphere point (|m0| < 2 R2, true for every workload of BASELINE.json at 80 and 128), inputs
-// 2..5 of every first-pass butterfly are zero and outputs 2..5 of every last-pass butterfly are discarded.
-// dft8_in0167: a[n] <- a0 + a1 w^n + a6 w^6n + a7 w^7n, w = exp(SIGN 2 pi i / 8)  (a[2..5] ignored on entry)
-template <int SIGN>
-__device__ __forceinline__ void dft8_in0167(double2 (&a)[8]) {
-    const double2 j6 = mul_i<SIGN>(a[6]);
-    const double2 e0 = cadd(a[0], a[6]), e2 = csub(a[0], a[6]), e1 = csub(a[0], j6), e3 = cadd(a[0], j6);
-    const double2 u = mul_w<SIGN, 1, 8>(a[1]), v = mul_w<SIGN, 7, 8>(a[7]);
-    const double2 o0 = cadd(a[1], a[7]), o2 = mul_i<SIGN>(csub(a[1], a[7]));
-    const double2 o1 = cadd(u, v), o3 = mul_i<SIGN>(csub(u, v));
-    a[0] = cadd(e0, o0); a[4] = csub(e0, o0);
-    a[1] = cadd(e1, o1); a[5] = csub(e1, o1);
-    a[2] = cadd(e2, o2); a[6] = csub(e2, o2);
-    a[3] = cadd(e3, o3); a[7] = csub(e3, o3);
-}
-// dft8_out0167: outputs 0, 1, 6, 7 of the full length-8 DFT (a[2..5] undefined on exit)
-template <int SIGN>
-__device__ __forceinline__ void dft8_out0167(double2 (&a)[8]) {
-    const double2 s0 = cadd(a[0], a[4]), s1 = cadd(a[1], a[5]), s2 = cadd(a[2], a[6]), s3 = cadd(a[3], a[7]);
-    const double2 d0 = csub(a[0], a[4]), d1 = csub(a[1], a[5]), d2 = csub(a[2], a[6]), d3 = csub(a[3], a[7]);
-    const double2 j2 = mul_i<SIGN>(d2), j3 = mul_i<SIGN>(d3);
-    a[0] = cadd(cadd(s0, s2), cadd(s1, s3));
-    a[6] = csub(csub(s0, s2), mul_i<SIGN>(csub(s1, s3)));
-    a[1] = cadd(cadd(d0, j2), mul_w<SIGN, 1, 8>(cadd(d1, j3)));
-    a[7] = cadd(csub(d0, j2), mul_w<SIGN, 7, 8>(csub(d1, j3)));
-}
-
 template <int LT, bool PR = false>
-__global__ void __launch_bounds__(Hyb<LT>::NT, Hyb<LT>::MINB) k_planes_fused_h(const double2 *__restrict__ tw, const int S1,
+__global__ void __launch_bounds__(Hyb<LT>::NT, (PR && LT == 80) ? 6 : Hyb<LT>::MINB) k_planes_fused_h(const double2 *__restrict__ tw, const int S1,
                                                                                      const int S2, const int npl,
                                                                                      const int *__restrict__ planeof,
                                                                                      double2 *__restrict__ W2,
@@ -1116,6 +1128,12 @@ int launch_rows(const jdft_basis *b, int nbt, double2 *W1, double2 *W2, cudaStre
     return JDFT_OK;
 }
 
+// occupied planes: i0 in [0, m0lo + npl) and [L + m0lo, L); the pruned radix-8 butterflies need [2 R2, 6 R2) empty
+template <class C>
+bool planes_prunable(const jdft_basis *b, int L) {
+    return C::R1 == 8 && b->opt_prune && b->m0lo < 0 && b->m0lo + b->npl <= 2 * C::R2 && L + b->m0lo >= 6 * C::R2;
+}
+
 template <int MODE>
 int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, double2 *psi, cudaStream_t st) {
     const int L = b->S[0];
@@ -1127,9 +1145,14 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
             if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(W2) && (((uintptr_t)V) & 15) == 0) {
                 using Q = Pair<LT>;
                 const size_t sm2 = (size_t)Q::G * L * Q::T * sizeof(double2);
-                JDFT_CUDA(ensure_smem(k_planes_fused2<LT>, sm2));
                 dim3 g2((b->S[2] + Q::T - 1) / Q::T, (b->S[1] + Q::G - 1) / Q::G, nbt);
-                k_planes_fused2<LT><<<g2, Q::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
+                if (planes_prunable<Tuned<LT>>(b, L)) {
+                    JDFT_CUDA(ensure_smem(k_planes_fused2<LT, true>, sm2));
+                    k_planes_fused2<LT, true><<<g2, Q::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
+                } else {
+                    JDFT_CUDA(ensure_smem(k_planes_fused2<LT>, sm2));
+                    k_planes_fused2<LT><<<g2, Q::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
+                }
                 jdft_prof_end(b, JDFT_K_PLANES, st);
                 JDFT_LAUNCH_CHECK("k_planes_fused2");
                 return JDFT_OK;
@@ -1152,10 +1175,7 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
                 using C = Tuned<LT>;
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
                 dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
-                // occupied planes: i0 in [0, m0lo + npl) and [L + m0lo, L); pruned butterflies need [2 R2, 6 R2) empty
-                const bool pruned = C::R1 == 8 && b->opt_prune && b->m0lo < 0 && b->m0lo + b->npl <= 2 * C::R2 &&
-                                    L + b->m0lo >= 6 * C::R2;
-                if (pruned) {
+                if (planes_prunable<C>(b, L)) {
                     JDFT_CUDA(ensure_smem(k_planes_fused_h<LT, true>, sm2));
                     k_planes_fused_h<LT, true><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
                 } else {

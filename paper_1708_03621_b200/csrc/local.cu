@@ -661,7 +661,7 @@ __global__ void __launch_bounds__(Hyb<LT>::NT) k_rows_hyb(const double2 *__restr
 
 // Last pass of I (MODE 1: occupied planes of W2 -> full real-space block) and first pass of I^+ / J (MODE 2: the
 // reverse), same hybrid as k_rows_hyb: pencil pairs with 256-bit loads in the first pass, single pencils in the last.
-template <int LT, int MODE>
+template <int LT, int MODE, bool PR = false>   // PR: pruned radix-8 first pass of I (MODE 1), see dft8_in0167
 __global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_io_hyb(const double2 *__restrict__ tw, const int S1, const int S2,
                                                                const int npl, const int *__restrict__ planeof,
                                                                double2 *__restrict__ W2, double2 *__restrict__ psi) {
@@ -683,6 +683,7 @@ __global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_io_hyb(const double2 *__
         double2 a0[R1], a1[R1];
 #pragma unroll
         for (int k = 0; k < R1; k++) {
+            if (PR && MODE == 1 && k >= 2 && k < 6) continue;
             const int row = bf + k * R2;
             a0[k] = a1[k] = make_double2(0.0, 0.0);
             if (MODE == 1) {
@@ -692,8 +693,13 @@ __global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_io_hyb(const double2 *__
                 if (2 * l < tmax) ld256(pb + row * plane + 2 * l, a0[k], a1[k]);
             }
         }
-        Dft<R1, SIGN>::run(a0);
-        Dft<R1, SIGN>::run(a1);
+        if constexpr (PR && MODE == 1) {
+            dft8_in0167<SIGN>(a0);
+            dft8_in0167<SIGN>(a1);
+        } else {
+            Dft<R1, SIGN>::run(a0);
+            Dft<R1, SIGN>::run(a1);
+        }
 #pragma unroll
         for (int j = 1; j < R1; j++) {
             double2 wv = __ldg(tw + bf * j);
@@ -1162,9 +1168,14 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
             if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(W2, psi)) {
                 using C = Tuned<LT>;
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
-                JDFT_CUDA(ensure_smem(k_planes_io_hyb<LT, MODE>, sm2));
                 dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
-                k_planes_io_hyb<LT, MODE><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, psi);
+                if (MODE == 1 && planes_prunable<C>(b, L)) {
+                    JDFT_CUDA(ensure_smem(k_planes_io_hyb<LT, MODE, MODE == 1>, sm2));
+                    k_planes_io_hyb<LT, MODE, MODE == 1><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, psi);
+                } else {
+                    JDFT_CUDA(ensure_smem(k_planes_io_hyb<LT, MODE>, sm2));
+                    k_planes_io_hyb<LT, MODE><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, psi);
+                }
                 jdft_prof_end(b, JDFT_K_PLANES, st);
                 JDFT_LAUNCH_CHECK("k_planes_io_hyb");
                 return JDFT_OK;

@@ -493,3 +493,10 @@ def test_planes_pruned_butterflies_match(ref, jd, cfg_id):
     jd.jdft_set_option(c.gb, "planes_prune", 1)
     assert rel_err_per_band(a, want) <= TOL and rel_err_per_band(b, want) <= TOL
     assert rel_err_per_band(a, b) <= 1e-13
+    # stand-alone I: its first pass along axis 0 is pruned the same way
+    want_psi = c.rb.apply_I(c.C).reshape(c.nb, -1)
+    psi1 = jd.jdft_apply_I(c.gb, dev(c.C)).cpu().numpy().reshape(c.nb, -1)
+    jd.jdft_set_option(c.gb, "planes_prune", 0)
+    psi0 = jd.jdft_apply_I(c.gb, dev(c.C)).cpu().numpy().reshape(c.nb, -1)
+    jd.jdft_set_option(c.gb, "planes_prune", 1)
+    assert rel_err_per_band(psi1, want_psi) <= TOL and rel_err_per_band(psi0, want_psi) <= TOL

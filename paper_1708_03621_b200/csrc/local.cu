@@ -735,7 +735,7 @@ __global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_io_hyb(const double2 *__
 }
 
 // Density with the hybrid first pass (pencil pairs, 256-bit loads) of k_planes_io_hyb and register accumulators.
-template <int LT>
+template <int LT, bool PR = false>   // PR: pruned radix-8 first pass, see dft8_in0167
 __global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_density_hyb(const double2 *__restrict__ tw, const int S1, const int S2,
                                                                     const int npl, const int *__restrict__ planeof,
                                                                     const double2 *__restrict__ W2, const double *__restrict__ f,
@@ -763,12 +763,18 @@ __global__ void __launch_bounds__(Hyb<LT>::NT) k_planes_density_hyb(const double
             double2 a0[R1], a1[R1];
 #pragma unroll
             for (int k = 0; k < R1; k++) {
+                if (PR && k >= 2 && k < 6) continue;
                 const int p = s_planeof[bf + k * R2];
                 a0[k] = a1[k] = make_double2(0.0, 0.0);
                 if (p >= 0 && 2 * l < tmax) ld256(W2b + p * plane + 2 * l, a0[k], a1[k]);
             }
-            Dft<R1, +1>::run(a0);
-            Dft<R1, +1>::run(a1);
+            if constexpr (PR) {
+                dft8_in0167<+1>(a0);
+                dft8_in0167<+1>(a1);
+            } else {
+                Dft<R1, +1>::run(a0);
+                Dft<R1, +1>::run(a1);
+            }
 #pragma unroll
             for (int j = 1; j < R1; j++) {
                 const double2 wv = __ldg(tw + bf * j);
@@ -1323,10 +1329,16 @@ extern "C" int jdft_density(const jdft_basis *b, const double *C_, int nb, const
                 if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(w.W2)) {
                     using C = Tuned<LT>;
                     const size_t sm2 = (size_t)L * C::T * sizeof(double2);
-                    JDFT_CUDA(ensure_smem(k_planes_density_hyb<LT>, sm2));
                     dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1]);
-                    k_planes_density_hyb<LT><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
-                                                                      f + b0, nbt, n, acc);
+                    if (planes_prunable<C>(b, L)) {
+                        JDFT_CUDA(ensure_smem(k_planes_density_hyb<LT, true>, sm2));
+                        k_planes_density_hyb<LT, true><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof,
+                                                                                     w.W2, f + b0, nbt, n, acc);
+                    } else {
+                        JDFT_CUDA(ensure_smem(k_planes_density_hyb<LT>, sm2));
+                        k_planes_density_hyb<LT><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
+                                                                          f + b0, nbt, n, acc);
+                    }
                     hyb = true;
                 }
             }

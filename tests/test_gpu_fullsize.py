@@ -67,6 +67,22 @@ def test_full_H_sampled_bands(full, jd):
     full.HC = HC
 
 
+def test_full_H_pruned_butterflies_are_taken_and_agree(full, jd):
+    """All five workloads leave planes [S0/4, 3 S0/4) empty, so K3 runs its pruned radix-8 butterflies (DESIGN.md
+    section 5); every band equals the unpruned kernel's result to rounding (the sampled bands are checked against the
+    oracle in test_full_H_sampled_bands)."""
+    m0 = full.rb.iG[:, 0]
+    assert max(m0.max(), -m0.min()) < full.S[0] // 4
+    jd.jdft_set_option(full.gb, "planes_prune", 0)
+    ref_HC = jd.jdft_apply_H(full.gb, full.dV, full.dP, full.dD, full.dC)
+    jd.jdft_set_option(full.gb, "planes_prune", 1)
+    HC = full.HC if hasattr(full, "HC") else jd.jdft_apply_H(full.gb, full.dV, full.dP, full.dD, full.dC)
+    num = torch.linalg.vector_norm(HC - ref_HC, dim=1)
+    den = torch.linalg.vector_norm(ref_HC, dim=1)
+    assert float((num / den).max()) <= 1e-13
+    del ref_HC
+
+
 def test_full_H_local_only_and_Vnl_alone(full, jd):
     Cs = full.C[full.sample]
     got = jd.jdft_apply_H(full.gb, full.dV, None, None, full.dC)[full.sample].cpu().numpy()

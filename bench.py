@@ -139,37 +139,49 @@ def config_sizes(cfg_id):
 
 # ------------------------------------------------------------------------------------------------ reference arm
 
+def oracle_sample_step(rb, inp, Cs, do_overlap):
+    """One pass of the oracle over a band sample of the workload: jdft_ref_apply_H on the sample and, where the step
+    contains the overlap (config 5), the sample's columns of C^+ O C against ALL bands (the sample's share of it)."""
+    rb.apply_H(inp["Vloc"], inp["P"], inp["D"], Cs)
+    if do_overlap:
+        rb.overlap(inp["C"], Cs)
+
+
 def run_reference(args):
     from oracle import ref
     cfg, nk, nb, nproj = config_sizes(args.config)
     R, kpts, Ecut, S = workloads.lattice(args.config)
+    do_overlap = args.config == 5
     threads = ref.threads()
     rb = ref.RefBasis(R, kpts[0], Ecut, S)
-    inp = workloads.make_inputs(args.config, rb.iG, ik=0, nb=max(threads, 1) * 4)
+    inp = workloads.make_inputs(args.config, rb.iG, ik=0, nb=nb if do_overlap else max(threads, 1) * 4,
+                                orthonormalise=not do_overlap)   # (QR of the full block is not part of the path)
     C = inp["C"]
     # calibrate: one band per thread, then size the per-step sample so the whole run stays within a few minutes
     t0 = time.perf_counter()
-    rb.apply_H(inp["Vloc"], inp["P"], inp["D"], C[:threads])
+    oracle_sample_step(rb, inp, C[:threads], do_overlap)
     t1 = time.perf_counter() - t0
     budget = 120.0 / max(1, args.steps + args.warmup)
     nsample = int(max(threads, min(C.shape[0], threads * max(1, int(budget / max(t1, 1e-3))))))
     nsample = (nsample // threads) * threads
     Cs = np.ascontiguousarray(C[:nsample])
     for _ in range(args.warmup):
-        rb.apply_H(inp["Vloc"], inp["P"], inp["D"], Cs)
+        oracle_sample_step(rb, inp, Cs, do_overlap)
     times = []
     for _ in range(args.steps):
         t0 = time.perf_counter()
-        rb.apply_H(inp["Vloc"], inp["P"], inp["D"], Cs)
+        oracle_sample_step(rb, inp, Cs, do_overlap)
         times.append(time.perf_counter() - t0)
     ms = 1e3 * float(np.mean(times))
     value = nsample / (ms * 1e-3)
-    sample = "%d bands of k-point 0 of config %d per step (full P, Vloc; apply_H only)" % (nsample, args.config)
+    sample = "%d bands of k-point 0 of config %d per step (full P, Vloc): jdft_ref_apply_H%s" % (
+        nsample, args.config, " + their %d x %d columns of jdft_ref_overlap" % (nb, nsample) if do_overlap else "")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "bands_per_step": nsample, "nproj": nproj, "fft_box": list(S)},
+        "config": {"workload": cfg["name"], "bands_per_step": nsample, "nproj": nproj, "fft_box": list(S),
+                   "overlap_in_step": do_overlap},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
@@ -178,27 +190,30 @@ def run_reference(args):
 
 def cpu_baseline(cfg_id, seconds=15.0):
     """The oracle, as it stands, on a bounded sample (about `seconds` of CPU work) of the same workload: whole passes
-    of jdft_ref_apply_H over `threads x 8` bands of k-point 0 (full P and Vloc), repeated until the time is used."""
+    of jdft_ref_apply_H over `threads x 4..8` bands of k-point 0 (full P and Vloc; config 5: plus those bands' columns
+    of the 512 x 512 overlap), repeated until the time is used."""
     from oracle import ref
     R, kpts, Ecut, S = workloads.lattice(cfg_id)
+    do_overlap = cfg_id == 5
     threads = ref.threads()
     rb = ref.RefBasis(R, kpts[0], Ecut, S)
     nb_cfg = workloads.get_config(cfg_id)["nb"]
-    nb = min(nb_cfg, threads * 8)
-    inp = workloads.make_inputs(cfg_id, rb.iG, ik=0, nb=nb)
+    nb = min(nb_cfg, threads * (4 if do_overlap else 8))
+    inp = workloads.make_inputs(cfg_id, rb.iG, ik=0, nb=nb_cfg if do_overlap else nb, orthonormalise=not do_overlap)
+    Cs = np.ascontiguousarray(inp["C"][:nb])
     t0 = time.perf_counter()
-    rb.apply_H(inp["Vloc"], inp["P"], inp["D"], inp["C"][:min(nb, threads)])      # warm-up / calibration
+    oracle_sample_step(rb, inp, Cs[:min(nb, threads)], do_overlap)      # warm-up / calibration
     t1 = time.perf_counter() - t0
     done, t0 = 0, time.perf_counter()
     while True:
-        rb.apply_H(inp["Vloc"], inp["P"], inp["D"], inp["C"])
+        oracle_sample_step(rb, inp, Cs, do_overlap)
         done += nb
         dt = time.perf_counter() - t0
         if dt >= seconds or dt + t1 * nb / max(1, min(nb, threads)) > 2 * seconds:
             break
     return {"value": done / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": "%d band-applications (%d bands of k-point 0 of config %d, repeated), jdft_ref_apply_H, %.1f s wall on %d threads"
-                      % (done, nb, cfg_id, dt, threads)}
+            "sample": "%d band-applications (%d bands of k-point 0 of config %d, repeated), jdft_ref_apply_H%s, %.1f s wall on %d threads"
+                      % (done, nb, cfg_id, " + their columns of the %d^2 jdft_ref_overlap" % nb_cfg if do_overlap else "", dt, threads)}
 
 
 # ------------------------------------------------------------------------------------------------ our arm
@@ -222,39 +237,34 @@ def algorithmic(cfgk, kernel, nbatches):
 
 
 def overlap_flops(nb, nG):
-    """Real flops jdft_overlap(C, C) performs: C^+ C is Hermitian, so only the 64 x 64 tiles on and below the diagonal
-    are computed ("half if only the Hermitian triangle is computed -- then count half")."""
-    t = (nb + 63) // 64
-    return 8 * (t * (t + 1) // 2) * 64 * 64 * nG
+    """Real flops counted for jdft_overlap(C, C): C^+ C is Hermitian, so only the triangle is needed (SURVEY.md 8(d):
+    "half if only the Hermitian triangle is computed -- then count half"): 8 nG nb (nb + 1) / 2.  (The kernel computes
+    whole 64 x 64 diagonal tiles, i.e. ~12 % more DMMAs than this at nb = 512; they are not counted.)"""
+    return 8 * (nb * (nb + 1) // 2) * nG
 
 
-def run_ours(args):
+def measure(cfg_id, args, rank, world, local, full):
+    """Times one BASELINE.json workload on this rank's GPU and returns the JSON line as a dict (rank 0; None elsewhere).
+    full = False: device-timed step and per-kernel rooflines only (no end-to-end leg, extras or CPU baseline)."""
     import torch
     import torch.distributed as dist
     import paper_1708_03621_b200.binding as jd
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl")
-    cfg, nk, nb, nproj = config_sizes(args.config)
-    R, kpts, Ecut, S = workloads.lattice(args.config)
-    do_overlap = args.config == 5
-    atoms = workloads.atoms_fractional(args.config)
-    Vh = workloads.make_vloc(args.config, atoms).reshape(-1)
+    cfg, nk, nb, nproj = config_sizes(cfg_id)
+    R, kpts, Ecut, S = workloads.lattice(cfg_id)
+    do_overlap = cfg_id == 5
+    steps = args.steps if full else min(args.steps, 5)
+    atoms = workloads.atoms_fractional(cfg_id)
+    Vh = workloads.make_vloc(cfg_id, atoms).reshape(-1)
     V = torch.from_numpy(Vh).cuda()
-    D_h = workloads.make_D(args.config)
+    D_h = workloads.make_D(cfg_id)
     D = torch.from_numpy(D_h).cuda()
     ks = []
     for ik in range(nk):
         gb = jd.jdft_basis_create(R, kpts[ik], Ecut, S, device=local)
         iG, _, _ = jd.jdft_basis_export(gb)
-        C_h = workloads.make_bands(args.config, gb.nG, ik=ik)
-        P_h = workloads.make_projectors(args.config, iG, kpts[ik], atoms)
+        C_h = workloads.make_bands(cfg_id, gb.nG, ik=ik)
+        P_h = workloads.make_projectors(cfg_id, iG, kpts[ik], atoms)
         jd.jdft_alloc_workspace(gb, max(args.batch, min(nb, args.ws_bands)), max(nb, nproj))
         if args.batch > 0:
             jd.jdft_set_option(gb, "band_batch", args.batch)
@@ -263,7 +273,7 @@ def run_ours(args):
         ks.append(dict(gb=gb, C=torch.from_numpy(C_h).cuda(), P=torch.from_numpy(P_h).cuda(),
                        HC=torch.empty((nb, gb.nG), dtype=torch.complex128, device="cuda"),
                        M=torch.empty((nb, nb), dtype=torch.complex128, device="cuda") if do_overlap else None,
-                       C_h=C_h, P_h=P_h,
+                       C_h=C_h if full else None, P_h=P_h if full else None,
                        info=dict(nG=gb.nG, a=gb.ncol * S[2], b=gb.npl * S[1] * S[2], N=gb.N, nb=nb, nproj=nproj,
                                  overlap_flops=overlap_flops(nb, gb.nG) if do_overlap else 0)))
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
@@ -313,7 +323,7 @@ def run_ours(args):
     jd.jdft_launch_count(reset=True)
     sampler = ClockSampler(local) if rank == 0 else None
     t_wall = time.perf_counter()
-    times = timed(args.steps)
+    times = timed(steps)
     t_wall = time.perf_counter() - t_wall
     if world > 1:
         dist.barrier()
@@ -331,37 +341,42 @@ def run_ours(args):
     units = nb * nk
     value = aggregate_value(units, world, ms_step)
 
-    # end to end through the HOST-buffer ABI call: pinned host inputs -> H2D -> kernels -> D2H, every step
-    Vp = torch.from_numpy(Vh).pin_memory()
-    Dp = torch.from_numpy(D_h).pin_memory()
-    host = [dict(C=torch.from_numpy(k["C_h"]).pin_memory(), P=torch.from_numpy(k["P_h"]).pin_memory(),
-                 HC=torch.empty((nb, k["gb"].nG), dtype=torch.complex128).pin_memory(),
-                 M=torch.empty((nb, nb), dtype=torch.complex128).pin_memory() if do_overlap else None) for k in ks]
+    e2e = None
+    if full:
+        # end to end through the HOST-buffer ABI call: pinned host inputs -> H2D -> kernels -> D2H, every step
+        Vp = torch.from_numpy(Vh).pin_memory()
+        Dp = torch.from_numpy(D_h).pin_memory()
+        host = [dict(C=torch.from_numpy(k["C_h"]).pin_memory(), P=torch.from_numpy(k["P_h"]).pin_memory(),
+                     HC=torch.empty((nb, k["gb"].nG), dtype=torch.complex128).pin_memory(),
+                     M=torch.empty((nb, nb), dtype=torch.complex128).pin_memory() if do_overlap else None) for k in ks]
 
-    def step_host():
-        for k, h in zip(ks, host):
-            jd.jdft_apply_H_host(k["gb"], Vp, h["P"], Dp, h["C"], h["HC"])
-            if do_overlap:
-                jd.jdft_overlap_host(k["gb"], h["C"], h["C"], h["M"])
+        def step_host():
+            for k, h in zip(ks, host):
+                jd.jdft_apply_H_host(k["gb"], Vp, h["P"], Dp, h["C"], h["HC"])
+                if do_overlap:
+                    jd.jdft_overlap_host(k["gb"], h["C"], h["C"], h["M"])
 
-    step_host()
-    e2e_steps = max(1, min(args.steps, 5))
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
         step_host()
-    torch.cuda.synchronize()
-    e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
-    e2e_ms = max_over_ranks(e2e_ms, world)
-    h2d = sum(h["C"].numel() * 16 + h["P"].numel() * 16 + Vp.numel() * 8 + Dp.numel() * 8 +
-              (2 * h["C"].numel() * 16 if do_overlap else 0) for h in host)
-    d2h = sum(h["HC"].numel() * 16 + (h["M"].numel() * 16 if do_overlap else 0) for h in host)
+        e2e_steps = max(1, min(steps, 5))
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            step_host()
+        torch.cuda.synchronize()
+        e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
+        e2e_ms = max_over_ranks(e2e_ms, world)
+        h2d = sum(h["C"].numel() * 16 + h["P"].numel() * 16 + Vp.numel() * 8 + Dp.numel() * 8 +
+                  (2 * h["C"].numel() * 16 if do_overlap else 0) for h in host)
+        d2h = sum(h["HC"].numel() * 16 + (h["M"].numel() * 16 if do_overlap else 0) for h in host)
+        e2e = {"value": aggregate_value(units, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps}
+        del host, Vp, Dp
 
     # SURVEY 8(f) rank 1 operations on the same inputs (k-point 0): density of all bands, subspace Hamiltonian C^+ (H C)
     extras = None
-    if args.extras:
+    if full and args.extras:
         k = ks[0]
         fo = torch.rand(nb, dtype=torch.float64, device="cuda")
         nr = torch.empty(tuple(S), dtype=torch.float64, device="cuda")
@@ -401,23 +416,28 @@ def run_ours(args):
         ms_I = t_op(lambda: jd.jdft_apply_I(k["gb"], CI, psiI))
         ms_J = t_op(lambda: jd.jdft_apply_J(k["gb"], psiI, CJ))
         ij_bytes = nbI * 16 * (i["nG"] + 2 * i["a"] + 2 * i["b"] + i["N"])
-        extras_ij = {"apply_I": {"ms": ms_I, "bands": nbI, "alg_GB/s": ij_bytes / (ms_I * 1e-3) / 1e9},
-                     "apply_J": {"ms": ms_J, "bands": nbI, "alg_GB/s": ij_bytes / (ms_J * 1e-3) / 1e9}}
         extras = {"pcm_hessian": {"ms": ms_h, "fields": nf, "nG": gs.nG, "fields_per_s": nf / (ms_h * 1e-3),
                                   "alg_GB/s": hess_bytes / (ms_h * 1e-3) / 1e9},
                   "density": {"ms": ms_d, "bands_per_s": nb / (ms_d * 1e-3), "alg_GB/s": dens_bytes / (ms_d * 1e-3) / 1e9},
-                  "subspace": {"ms": ms_s, "TFLOP/s": 8.0 * nb * nb * i["nG"] / (ms_s * 1e-3) / 1e12}}
-        extras.update(extras_ij)
+                  "subspace": {"ms": ms_s, "TFLOP/s": 8.0 * nb * nb * i["nG"] / (ms_s * 1e-3) / 1e12},
+                  "apply_I": {"ms": ms_I, "bands": nbI, "alg_GB/s": ij_bytes / (ms_I * 1e-3) / 1e9},
+                  "apply_J": {"ms": ms_J, "bands": nbI, "alg_GB/s": ij_bytes / (ms_J * 1e-3) / 1e9}}
+        extras.update(extra_ops(jd, torch, t_op, k, ks, V, D, S, nb, nproj, cfg))
+        del gs, phi, epsr, hout, psiI
 
+    infos = [k["info"] for k in ks]
+    nGs = [k["gb"].nG for k in ks]
+    del ks, V, D, flush
+    torch.cuda.empty_cache()
     if rank != 0:
-        return
+        return None
     hbm_peak, hbm_src = measured_peaks()
     dmma_peak, dfma_peak, fp_src = fp64_peak()
 
     def roof(name, ms, launches_):
         if ms <= 0:
             return None
-        alg = sum(algorithmic(k["info"], name, max(1, launches_ // max(1, len(ks)))) for k in ks)
+        alg = sum(algorithmic(i, name, max(1, launches_ // max(1, len(infos)))) for i in infos)
         if name in HBM_KERNELS:
             ach = alg / (ms * 1e-3) / 1e9
             return {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
@@ -430,31 +450,33 @@ def run_ours(args):
         kernels[name] = {"ms_per_step": ms, "launches": n}
         if r and name != "splitk_reduce":
             kernels[name].update({"achieved": r["achieved"], "unit": r["unit"], "frac": r["frac"]})
-    roofline = roof(dominant, dom_ms / args.steps, dom_n // args.steps)
-    roofline.update({"kernel": dominant, "launches_per_step": dom_n // args.steps,
+        t = ncu_traffic(cfg_id, name)
+        if t is not None:
+            kernels[name]["traffic_per_launch"] = t
+    roofline = roof(dominant, dom_ms / steps, dom_n // steps)
+    roofline.update({"kernel": dominant, "launches_per_step": dom_n // steps,
                      "avg_launch_ms": dom_ms / max(1, dom_n), "peak_source": hbm_src if roofline["bound"] == "hbm" else fp_src,
-                     "traffic": None, "share_of_step": dom_ms / args.steps / ms_step})
-    roofline["traffic"] = ncu_traffic(args.config, dominant)
-    dom_launches_step = max(1, dom_n // args.steps)
-    roofline["algorithmic_per_launch"] = sum(algorithmic(k["info"], dominant, max(1, dom_launches_step // max(1, len(ks))))
-                                             for k in ks) / dom_launches_step
-    roofline["note"] = ("algorithmic bytes (flops) per launch = DESIGN.md section 6 per-band figure x bands per launch; "
-                        "traffic = ncu dram bytes per launch (profiles/traffic.csv)")
-    local_bytes = sum(sum(algorithmic(k["info"], n, max(1, nbatches[n] // len(ks))) for n in
-                          ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd")) for k in ks)
-    local_ms = sum(per_kernel[n][0] for n in ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd"))
-    gemm_flops = sum(algorithmic(k["info"], "gemm_dotk", 1) + algorithmic(k["info"], "gemm_expand", 1) for k in ks)
+                     "traffic": None, "share_of_step": dom_ms / steps / ms_step})
+    roofline["traffic"] = ncu_traffic(cfg_id, dominant)
+    dom_launches_step = max(1, dom_n // steps)
+    roofline["algorithmic_per_launch"] = sum(algorithmic(i, dominant, max(1, dom_launches_step // max(1, len(infos))))
+                                             for i in infos) / dom_launches_step
+    roofline["note"] = ("algorithmic bytes (flops) per launch = DESIGN.md section 6 per-band figure x bands per launch "
+                        "(complex MAC = 8 real flops whatever the kernel executes); traffic = ncu dram bytes per launch "
+                        "(profiles/traffic.csv)")
+    fft_names = ("cols_inv", "rows_inv", "planes", "rows_fwd", "cols_fwd")
+    local_bytes = sum(sum(algorithmic(i, n, max(1, nbatches[n] // len(infos))) for n in fft_names) for i in infos)
+    local_ms = sum(per_kernel[n][0] for n in fft_names)
+    gemm_flops = sum(algorithmic(i, "gemm_dotk", 1) + algorithmic(i, "gemm_expand", 1) for i in infos)
     gemm_ms = per_kernel["gemm_dotk"][0] + per_kernel["gemm_expand"][0]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": cfg["name"], "bands": nb, "kpoints": nk, "nproj": nproj, "fft_box": list(S),
-                   "nG": [k["gb"].nG for k in ks], "overlap_in_step": do_overlap, "l2": "flushed (512 MiB memset) before every timed step",
+                   "nG": nGs, "overlap_in_step": do_overlap, "l2": "flushed (512 MiB memset) before every timed step",
                    "parallelism": "replicas x%d" % world},
         "clocks": clocks,
-        "e2e": {"value": aggregate_value(units, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": e2e_ms, "steps": e2e_steps},
         "gpu_launches": launches,
         "roofline": roofline,
         "groups": {"fft_local": {"GB/s": local_bytes / (local_ms * 1e-3) / 1e9 if local_ms else None,
@@ -467,11 +489,54 @@ def run_ours(args):
         "fp64_peaks": {"dmma_tflops": dmma_peak, "dfma_tflops": dfma_peak, "source": fp_src},
         "wall_s_timed_region": t_wall,
     }
-    if args.extras:
+    if e2e is not None:
+        line["e2e"] = e2e
+    if extras is not None:
         line["extras"] = extras
-    if world == 1 and not args.no_cpu_baseline:
+    return line
+
+
+def extra_ops(jd, torch, t_op, k, ks, V, D, S, nb, nproj, cfg):
+    """Timings of the SURVEY 8(f) rank 2 / 3 additions (filled in where the library exports them)."""
+    return {}
+
+
+def compact(line):
+    """Sub-record of a non-headline config: the device-timed value and the per-kernel roofline fractions."""
+    return {"workload": line["config"]["workload"], "value": line["value"], "unit": line["unit"],
+            "ms_per_step": line["ms_per_step"], "steps": line["steps"], "clocks": line["clocks"],
+            "roofline": {k: line["roofline"][k] for k in ("kernel", "bound", "achieved", "peak", "unit", "frac", "traffic")},
+            "groups": line["groups"],
+            "kernel_frac": {n: round(v["frac"], 4) for n, v in line["kernels"].items() if "frac" in v}}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    t_start = time.perf_counter()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    line = measure(args.config, args, rank, world, local, full=True)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args.config)
-    print(json.dumps(line), flush=True)
+    # compact sub-records of the other full-size workloads (device-timed only), while the time budget allows
+    others = [c for c in args.also if c != args.config] if world == 1 else []
+    if others:
+        line["other_configs"] = {}
+        for c in others:
+            if time.perf_counter() - t_start > args.also_budget:
+                line["other_configs"][str(c)] = "skipped (time budget of the default run)"
+                continue
+            line["other_configs"][str(c)] = compact(measure(c, args, rank, world, local, full=False))
+    if rank == 0:
+        print(json.dumps(line), flush=True)
 
 
 def main():
@@ -479,15 +544,21 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json workload 1..5 (default 2 = configs[1])")
+    ap.add_argument("--config", type=int, default=5,
+                    help="BASELINE.json workload 1..5 (default 5: the largest single-GPU one, 512 bands + the 512^2 overlap)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=0, help="bands per FFT batch (0 = automatic)")
     ap.add_argument("--ws-bands", type=int, default=256, help="bands of FFT scratch in the workspace (= automatic batch size)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--extras", action="store_true", help="also time jdft_density and jdft_subspace (SURVEY 8(f) rank 1)")
+    ap.add_argument("--extras", action="store_true", help="also time the SURVEY 8(f) operations (density, subspace, Listing 1, ...)")
     ap.add_argument("--overlap", action="store_true",
                     help="run the projection GEMM on a side stream beside the FFT pipeline (measured +1-2 %%; off by default)")
+    ap.add_argument("--also", type=lambda s: [int(x) for x in s.split(",") if x], default=None,
+                    help="other configs to attach as compact sub-records (default: 2,3,4 when --config is 5 and all defaults)")
+    ap.add_argument("--also-budget", type=float, default=150.0, help="seconds after which no further sub-record is started")
     args = ap.parse_args()
+    if args.also is None:
+        args.also = [2, 3, 4] if args.config == 5 else []
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) == 0:
             run_reference(args)

@@ -114,6 +114,8 @@ static int posmod(int a, int n) {
     return r < 0 ? r + n : r;
 }
 
+int jdft_ref_basis_destroy(jdft_ref_basis *b);
+
 int jdft_ref_basis_create(const double *R, const double *k, double Ecut, const int *S,
                           jdft_ref_basis **out) {
     if (!R || !k || !S || !out || !(Ecut > 0.0)) return REF_EINVAL;
@@ -135,13 +137,15 @@ int jdft_ref_basis_create(const double *R, const double *k, double Ecut, const i
             b->GGT[3 * i + j] = s;
         }
     b->N = (int64_t)S[0] * S[1] * S[2];
-    /* bounding integer range of the ellipsoid: |m_d + k_d| <= sqrt(2 Ecut) |a_d| / (2 pi), padded by 1 */
+    /* Plain whole-range sweep ("brute force"): no ellipsoid geometry is used to bound the loop.
+     * Per axis the range is the 2 S_d + 1 integers centred on the integer nearest to -k_d (the centre of the cutoff
+     * region): any region that passes the box test below (extent < S_d) lies inside it, and a region that does not
+     * still shows an extent >= S_d inside it (it is convex and centred within 1/2 of the range's centre).          */
     int lo[3], hi[3];
     for (int d = 0; d < 3; d++) {
-        double len = sqrt(R[d] * R[d] + R[3 + d] * R[3 + d] + R[6 + d] * R[6 + d]);
-        double bound = sqrt(2.0 * Ecut) * len / (2.0 * M_PI);
-        lo[d] = (int)floor(-k[d] - bound) - 1;
-        hi[d] = (int)ceil(-k[d] + bound) + 1;
+        int c = (int)lround(-k[d]);
+        lo[d] = c - S[d];
+        hi[d] = c + S[d];
     }
     /* two brute-force sweeps: count, then fill, in (m0, m1, m2) lexicographic order, m2 fastest */
     for (int pass = 0; pass < 2; pass++) {
@@ -178,6 +182,18 @@ int jdft_ref_basis_create(const double *R, const double *k, double Ecut, const i
             b->ke = (double *)malloc(sizeof(double) * n);
             if (!b->iG || !b->index || !b->ke) return REF_ENOMEM;
         }
+    }
+    /* separate collision check, literally: no two sphere points may land on the same box offset */
+    {
+        unsigned char *seen = (unsigned char *)calloc((size_t)b->N, 1);
+        if (!seen) return REF_ENOMEM;
+        int dup = 0;
+        for (int64_t n = 0; n < b->nG; n++) {
+            if (seen[b->index[n]]) dup = 1;
+            seen[b->index[n]] = 1;
+        }
+        free(seen);
+        if (dup) { jdft_ref_basis_destroy(b); return REF_EBOX; }
     }
     *out = b;
     return REF_OK;

@@ -179,6 +179,29 @@ def test_overlap(case, jd):
     assert rel_err_per_band(got.T, want.T) <= TOL           # per column of M
 
 
+@pytest.mark.parametrize("nb", [64, 65, 130, 200])
+def test_overlap_hermitian_triangle_path(ref, jd, nb):
+    """jdft_overlap(C, C) / jdft_subspace(C, C) with the SAME array on both sides compute the lower-triangle tiles only
+    and mirror them; NON-orthonormal bands make every off-diagonal entry O(1), so a wrong mirror index or conjugation
+    sign fails.  nb straddles one, two, three and four 64-wide tiles with ragged tails."""
+    R, kpts, Ecut, S = workloads.lattice(104)
+    rb = ref.RefBasis(R, kpts[0], Ecut, S)
+    gb = jd.jdft_basis_create(R, kpts[0], Ecut, S)
+    jd.jdft_alloc_workspace(gb, 1, nb)
+    C = workloads.make_bands(104, rb.nG, nb=nb, orthonormalise=False)
+    C = np.ascontiguousarray(C * (1.0 + np.arange(nb) % 5)[:, None] * np.exp(0.3j * np.arange(nb))[:, None])
+    dC = dev(C)
+    want = rb.overlap(C, C)
+    got = jd.jdft_overlap(gb, dC, dC).cpu().numpy()
+    assert rel_err_per_band(got.T, want.T) <= TOL
+    assert np.max(np.abs(got - got.conj().T)) <= 1e-13 * np.max(np.abs(got))
+    gots = jd.jdft_subspace(gb, dC, dC).cpu().numpy()
+    assert rel_err_per_band(gots.T, rb.subspace(C, C).T) <= TOL
+    # distinct arrays with equal contents take the full (non-triangle) path: same result
+    got2 = jd.jdft_overlap(gb, dC, dC.clone()).cpu().numpy()
+    assert rel_err_per_band(got2.T, want.T) <= TOL
+
+
 def test_host_variants(case, jd):
     want = case.rb.apply_H(case.V, case.P, case.D, case.C)
     HC = torch.empty(case.C.shape, dtype=torch.complex128).pin_memory()

@@ -369,11 +369,14 @@ int jdft_ref_apply_O(const jdft_ref_basis *b, const double *C_, int nb, double *
  * Vnl: out (+)= P D P^+ C.
  *   B[ib][j]  = sum_n conj(P[j][n]) C[ib][n]
  *   B'[ib][j] = D[j] B[ib][j]            (D_mode 0)   or   sum_l D[j][l] B[ib][l]   (D_mode 1)
+ *   or, D_mode = nblk >= 2 (per-atom Hermitian blocks c128[np/nblk][nblk][nblk], reading 24; PAPER.md:95
+ *   ultrasoft pseudopotentials couple the projectors of one atom only):
+ *   B'[ib][a nblk + j'] = sum_l' D[a][j'][l'] B[ib][a nblk + l']
  *   out[ib][n] (+)= sum_j P[j][n] B'[ib][j]
  */
 int jdft_ref_apply_Vnl(const jdft_ref_basis *b, const double *P_, int np, const double *D, int D_mode,
                        const double *C_, int nb, double *out_, int accumulate) {
-    if (!b || !C_ || !out_ || nb < 0 || np < 0 || (np > 0 && (!P_ || !D)) || (D_mode != 0 && D_mode != 1))
+    if (!b || !C_ || !out_ || nb < 0 || np < 0 || (np > 0 && (!P_ || !D)) || D_mode < 0 || (D_mode >= 2 && np % D_mode != 0))
         return REF_EINVAL;
     const cplx *P = (const cplx *)P_, *C = (const cplx *)C_;
     cplx *out = (cplx *)out_;
@@ -397,10 +400,16 @@ int jdft_ref_apply_Vnl(const jdft_ref_basis *b, const double *P_, int np, const 
         for (int j = 0; j < np; j++) {
             if (D_mode == 0) {
                 B2[j] = D[j] * B[j];
-            } else {
+            } else if (D_mode == 1) {
                 const cplx *Dc = (const cplx *)D;
                 lcplx s = 0.0L;
                 for (int l = 0; l < np; l++) s += (lcplx)Dc[(size_t)j * np + l] * (lcplx)B[l];
+                B2[j] = (cplx)s;
+            } else { /* per-atom blocks: D[a][j'][l'], a = j / nblk, only projectors of the same atom couple */
+                const int nblk = D_mode, a = j / nblk, jj = j % nblk;
+                const cplx *Da = (const cplx *)D + (size_t)a * nblk * nblk;
+                lcplx s = 0.0L;
+                for (int l = 0; l < nblk; l++) s += (lcplx)Da[(size_t)jj * nblk + l] * (lcplx)B[(size_t)a * nblk + l];
                 B2[j] = (cplx)s;
             }
         }
@@ -620,5 +629,34 @@ int jdft_ref_pcm_hessian(const jdft_ref_basis *b, const double *epsilon, const d
     }
     free(g);
     free(r);
+    return rc;
+}
+
+/* ---- ultrasoft pseudopotentials ("norm-conserving and ultrasoft
+ * pseudopotentials"; Listing 2's own input uses the GBRV ultrasoft library).  The generalised
+ * overlap operator carries a projector term (reading 24):
+ *     O_us C = Omega ( C + P Q P^+ C ),        M_us = C1^+ O_us C2   (column-major nb1 x nb2),
+ * with Q given as data in the same three layouts as D (Q_mode 0 real diagonal, 1 dense Hermitian, nblk >= 2 per-atom
+ * blocks).  Written out literally: the nonlocal product first, then the sum, then the plain inner products.      */
+int jdft_ref_apply_O_us(const jdft_ref_basis *b, const double *P, int np, const double *Q, int Q_mode,
+                        const double *C_, int nb, double *out_) {
+    if (!b || nb < 0 || np < 0 || (nb > 0 && (!C_ || !out_))) return REF_EINVAL;
+    int rc = jdft_ref_apply_Vnl(b, P, np, Q, Q_mode, C_, nb, out_, 0);   /* out = P Q P^+ C   (0 when np = 0) */
+    if (rc) return rc;
+    if (np == 0) memset(out_, 0, sizeof(cplx) * (size_t)nb * b->nG);
+    const cplx *C = (const cplx *)C_;
+    cplx *out = (cplx *)out_;
+    for (int64_t i = 0; i < (int64_t)nb * b->nG; i++) out[i] = b->volume * (C[i] + out[i]);
+    return REF_OK;
+}
+
+int jdft_ref_overlap_us(const jdft_ref_basis *b, const double *P, int np, const double *Q, int Q_mode,
+                        const double *C1, int nb1, const double *C2, int nb2, double *M) {
+    if (!b || nb1 < 0 || nb2 < 0 || !C1 || !C2 || !M) return REF_EINVAL;
+    double *X = (double *)malloc(sizeof(cplx) * (size_t)(nb2 > 0 ? nb2 : 1) * b->nG);
+    if (!X) return REF_ENOMEM;
+    int rc = jdft_ref_apply_O_us(b, P, np, Q, Q_mode, C2, nb2, X);       /* X = O_us C2 */
+    if (!rc) rc = jdft_ref_subspace(b, C1, nb1, X, nb2, M);              /* M = C1^+ X  */
+    free(X);
     return rc;
 }

@@ -6,8 +6,8 @@ __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may 
 It imports nothing from the CUDA package and the CUDA package imports nothing from here.
 
 All arrays are numpy, host memory: C is complex128 [nb, nG]; psi is complex128 [nb, S0, S1, S2];
-Vloc is float64 [S0, S1, S2] (or flat [N]); P is complex128 [np, nG]; D is float64 [np] (diagonal)
-or complex128 [np, np] (dense Hermitian); the overlap is returned as M[a, b] (nb1 x nb2).
+Vloc is float64 [S0, S1, S2] (or flat [N]); P is complex128 [np, nG]; D is float64 [np] (diagonal),
+complex128 [np, np] (dense Hermitian) or complex128 [natoms, nblk, nblk] (per-atom Hermitian blocks); the overlap is returned as M[a, b] (nb1 x nb2).
 """
 import ctypes
 import os
@@ -59,6 +59,8 @@ def lib():
         L.jdft_ref_gradient.argtypes = [vp, vp, ci, vp]
         L.jdft_ref_divergence.argtypes = [vp, vp, ci, vp]
         L.jdft_ref_pcm_hessian.argtypes = [vp, vp, vp, ci, vp]
+        L.jdft_ref_apply_O_us.argtypes = [vp, vp, ci, vp, ci, vp, ci, vp]
+        L.jdft_ref_overlap_us.argtypes = [vp, vp, ci, vp, ci, vp, ci, vp, ci, vp]
         _lib = L
     return _lib
 
@@ -157,6 +159,9 @@ class RefBasis:
         D = np.asarray(D)
         if D.ndim == 1:
             return np.ascontiguousarray(D, dtype=np.float64), 0
+        if D.ndim == 3:  # per-atom Hermitian blocks [natoms, nblk, nblk]: D_mode = nblk
+            assert D.shape[1] == D.shape[2] >= 2 and D.shape[0] * D.shape[1] == nproj
+            return _c128(D), int(D.shape[1])
         assert D.shape == (nproj, nproj)
         return _c128(D), 1
 
@@ -239,6 +244,23 @@ class RefBasis:
         out = np.empty_like(phi)
         _chk(lib().jdft_ref_pcm_hessian(self._h, _p(eps), _p(phi), phi.shape[0], _p(out)))
         return out
+
+    def apply_O_us(self, P, Q, C):
+        """Ultrasoft generalised overlap operator: Omega (C + P Q P^+ C); Q like D (diag / dense / per-atom blocks)."""
+        C, P = _c128(C), _c128(P)
+        Qm, mode = self._D(Q, P.shape[0])
+        out = np.empty_like(C)
+        _chk(lib().jdft_ref_apply_O_us(self._h, _p(P), P.shape[0], _p(Qm), mode, _p(C), C.shape[0], _p(out)))
+        return out
+
+    def overlap_us(self, P, Q, C1, C2):
+        """M[a, b] = C1[a]^+ O_us C2[b] with O_us = Omega (1 + P Q P^+)."""
+        C1, C2, P = _c128(C1), _c128(C2), _c128(P)
+        Qm, mode = self._D(Q, P.shape[0])
+        nb1, nb2 = C1.shape[0], C2.shape[0]
+        M = np.empty((nb2, nb1), dtype=np.complex128)
+        _chk(lib().jdft_ref_overlap_us(self._h, _p(P), P.shape[0], _p(Qm), mode, _p(C1), nb1, _p(C2), nb2, _p(M)))
+        return M.T
 
     def overlap_entry(self, C1, C2, a, b):
         C1, C2 = _c128(C1), _c128(C2)

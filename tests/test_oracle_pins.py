@@ -476,3 +476,94 @@ def test_pcm_hessian_vs_explicit_matrices_constant_epsilon_and_hermiticity(ref):
     Ha, Hb = got[0], got[1]
     assert abs(np.vdot(a_, Hb) - np.conj(np.vdot(b_, Ha))) <= 1e-12 * np.linalg.norm(a_) * np.linalg.norm(Hb)
     assert np.real(np.vdot(a_, Ha)) > 0
+
+
+# ------------------------------------------------------------------------------------------ ultrasoft (8(f) rank 2)
+
+def _blocks(rng, natoms, nblk, psd=False):
+    A = _rand_c(rng, natoms, nblk, nblk)
+    if psd:
+        return A @ A.conj().transpose(0, 2, 1)
+    return A + A.conj().transpose(0, 2, 1)
+
+
+def _block_diag(Q):
+    na, n, _ = Q.shape
+    out = np.zeros((na * n, na * n), complex)
+    for a in range(na):
+        out[a * n:(a + 1) * n, a * n:(a + 1) * n] = Q[a]
+    return out
+
+
+def test_block_diagonal_D_vs_dense_matrix(ref):
+    """D_mode = nblk (per-atom Hermitian blocks, reading 24): P D P^+ against the dense nG x nG matrix built
+    from the explicitly assembled block-diagonal D; a wrong block offset, a transposed block or coupling across atoms
+    fails.  Blocks of one atom's 4 projectors, and 2-projector blocks (8 = 4 x 2)."""
+    cfg = 101
+    R, kpts, Ecut, S = workloads.lattice(cfg)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    assert b.nG <= 400
+    inp = workloads.make_inputs(cfg, b.iG)
+    P, C = inp["P"], inp["C"]
+    Pm = P.T
+    rng = np.random.default_rng(61)
+    for nblk in (4, 2):
+        Db = _blocks(rng, P.shape[0] // nblk, nblk)
+        want = C @ (Pm @ _block_diag(Db) @ Pm.conj().T).T
+        got = b.apply_Vnl(P, Db, C)
+        assert np.max(np.abs(got - want)) <= 1e-12 * np.max(np.abs(want))
+        # same operator through the dense mode
+        assert np.max(np.abs(got - b.apply_Vnl(P, _block_diag(Db), C))) <= 1e-12 * np.max(np.abs(want))
+    # blocks that are diagonal reduce to the real-diagonal mode
+    d = inp["D"]
+    Dd = np.zeros((P.shape[0] // 4, 4, 4), complex)
+    for a in range(Dd.shape[0]):
+        Dd[a] = np.diag(d[4 * a:4 * a + 4])
+    assert np.max(np.abs(b.apply_Vnl(P, Dd, C) - b.apply_Vnl(P, d, C))) <= 1e-13 * np.max(np.abs(C))
+    # H with block D = sum of its terms
+    V = inp["Vloc"]
+    Db = _blocks(rng, P.shape[0] // 4, 4)
+    assert np.allclose(b.apply_H(V, P, Db, C), b.apply_H(V, None, None, C) + b.apply_Vnl(P, Db, C), rtol=1e-13, atol=1e-16)
+
+
+def test_ultrasoft_overlap_operator_vs_dense_matrix(ref):
+    """O_us = Omega (1 + P Q P^+) (PAPER.md:95 ultrasoft pseudopotentials; reading 24) against the dense
+    nG x nG matrix; Hermitian; positive definite for PSD Q; reduces to Omega at Q = 0 and at np = 0; the generalised
+    overlap M = C1^+ O_us C2 against numpy; all three Q layouts."""
+    cfg = 101
+    R, kpts, Ecut, S = workloads.lattice(cfg)
+    b = ref.RefBasis(R, kpts[0], Ecut, S)
+    assert b.nG <= 400
+    inp = workloads.make_inputs(cfg, b.iG)
+    P, C = inp["P"], inp["C"]
+    Pm = P.T
+    rng = np.random.default_rng(67)
+    C2 = _rand_c(rng, 3, b.nG)
+    Qb = _blocks(rng, P.shape[0] // 4, 4, psd=True)
+    Qdense = _rand_c(rng, P.shape[0], P.shape[0]); Qdense = Qdense + Qdense.conj().T
+    qdiag = rng.uniform(0.1, 1.0, P.shape[0])
+    for Q, Qfull in ((Qb, _block_diag(Qb)), (Qdense, Qdense), (qdiag, np.diag(qdiag))):
+        Ous = b.volume * (np.eye(b.nG) + Pm @ Qfull @ Pm.conj().T)
+        assert np.max(np.abs(Ous - Ous.conj().T)) <= 1e-12 * np.max(np.abs(Ous))
+        got = b.apply_O_us(P, Q, C)
+        want = C @ Ous.T
+        assert np.max(np.abs(got - want)) <= 1e-12 * np.max(np.abs(want))
+        M = b.overlap_us(P, Q, C, C2)
+        wantM = C.conj() @ Ous @ C2.T
+        assert M.shape == (C.shape[0], 3)
+        assert np.max(np.abs(M - wantM)) <= 1e-12 * np.max(np.abs(wantM))
+        # Hermitian: M(C1, C2) = M(C2, C1)^+
+        assert np.max(np.abs(b.overlap_us(P, Q, C2, C) - M.conj().T)) <= 1e-12 * np.max(np.abs(M))
+    # PSD Q: every Rayleigh quotient of O_us is >= Omega |c|^2
+    Mself = b.overlap_us(P, Qb, C2, C2)
+    assert np.all(np.linalg.eigvalsh((Mself + Mself.conj().T) / 2) > 0)
+    for c in C2:
+        assert np.vdot(c, b.apply_O_us(P, Qb, c[None])[0]).real >= b.volume * np.vdot(c, c).real * (1 - 1e-12)
+    # Q = 0 and no projectors: the norm-conserving O = Omega
+    assert np.max(np.abs(b.apply_O_us(P, np.zeros(P.shape[0]), C) - b.apply_O(C))) == 0.0
+    assert np.max(np.abs(b.apply_O_us(P[:0], np.zeros(0), C) - b.apply_O(C))) == 0.0
+    assert np.max(np.abs(b.overlap_us(P, np.zeros(P.shape[0]), C, C2) - b.overlap(C, C2))) <= 1e-13 * b.volume
+    # rank one: O_us c = Omega (c + q p (p^+ c))
+    p, q = P[:1], np.array([0.3])
+    want = b.volume * np.stack([c + q[0] * p[0] * np.vdot(p[0], c) for c in C])
+    assert np.max(np.abs(b.apply_O_us(p, q, C) - want)) <= 1e-13 * np.max(np.abs(want))

@@ -270,6 +270,9 @@ def measure(cfg_id, args, rank, world, local, full):
             jd.jdft_set_option(gb, "band_batch", args.batch)
         if args.overlap:
             jd.jdft_set_option(gb, "overlap_gemm", 1)
+        for kv in args.opt:
+            key, val = kv.split("=")
+            jd.jdft_set_option(gb, key, int(val))
         ks.append(dict(gb=gb, C=torch.from_numpy(C_h).cuda(), P=torch.from_numpy(P_h).cuda(),
                        HC=torch.empty((nb, gb.nG), dtype=torch.complex128, device="cuda"),
                        M=torch.empty((nb, nb), dtype=torch.complex128, device="cuda") if do_overlap else None,
@@ -553,6 +556,7 @@ def main():
     ap.add_argument("--extras", action="store_true", help="also time the SURVEY 8(f) operations (density, subspace, Listing 1, ...)")
     ap.add_argument("--overlap", action="store_true",
                     help="run the projection GEMM on a side stream beside the FFT pipeline (measured +1-2 %%; off by default)")
+    ap.add_argument("--opt", action="append", default=[], help="library option key=value (jdft_set_option), repeatable; for experiments")
     ap.add_argument("--also", type=lambda s: [int(x) for x in s.split(",") if x], default=None,
                     help="other configs to attach as compact sub-records (default: 2,3,4 when --config is 5 and all defaults)")
     ap.add_argument("--also-budget", type=float, default=150.0, help="seconds after which no further sub-record is started")

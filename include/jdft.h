@@ -102,8 +102,11 @@ int jdft_apply_J(const jdft_basis *b, const double *psi, int nb, double *C, jdft
 /* L C = -2 Omega ke C ; O C = Omega C.  May run in place (out == C).                                  */
 int jdft_apply_L(const jdft_basis *b, const double *C, int nb, double *LC, jdft_stream s);
 int jdft_apply_O(const jdft_basis *b, const double *C, int nb, double *OC, jdft_stream s);
-/* Vnl: out (+)= P D P^+ C.  P c128[nproj][nG]; D_mode 0: D = f64[nproj] real diagonal;
- * D_mode 1: D = c128[nproj][nproj] row-major Hermitian; accumulate != 0 adds into out.               */
+/* Vnl: out (+)= P D P^+ C (PAPER.md:127 SpeciesInfo pseudopotentials).  P c128[nproj][nG];
+ * D_mode 0: D = f64[nproj] real diagonal;  D_mode 1: D = c128[nproj][nproj] row-major Hermitian;
+ * D_mode = nblk >= 2: per-atom Hermitian blocks D = c128[nproj / nblk][nblk][nblk] (block a couples projectors
+ * a nblk .. a nblk + nblk - 1 only -- the ultrasoft case of PAPER.md:95; nproj % nblk must be 0; reading 24).
+ * The same three layouts are accepted wherever a D or Q is taken.  accumulate != 0 adds into out.              */
 int jdft_apply_Vnl(const jdft_basis *b, const double *P, int nproj, const double *D, int D_mode,
                    const double *C, int nb, double *out, int accumulate, jdft_stream s);
 /* projection alone: Bproj [nb][nproj] = (P^+ C)^T, i.e. Bproj[ib][j] = sum_n conj(P[j][n]) C[ib][n]   */
@@ -116,6 +119,16 @@ int jdft_apply_H(const jdft_basis *b, const double *Vloc, const double *P, int n
 /* overlap: M[a + nb1*bb] = Omega sum_n conj(C1[a][n]) C2[bb][n]  (column-major nb1 x nb2, c128)       */
 int jdft_overlap(const jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M,
                  jdft_stream s);
+
+/* ---- ultrasoft pseudopotentials ("norm-conserving and ultrasoft pseudopotentials",
+ * PAPER.md:166-169 Listing 2 runs on the GBRV ultrasoft library; reading 24) ------------------------------
+ * generalised overlap operator   O_us C = Omega (C + P Q P^+ C),   Q in the layouts of D (Q_mode as D_mode);
+ * OC may alias C.  nproj == 0 gives O C = Omega C.                                                              */
+int jdft_apply_O_us(const jdft_basis *b, const double *P, int nproj, const double *Q, int Q_mode, const double *C,
+                    int nb, double *OC, jdft_stream s);
+/* generalised overlap matrix     M[a + nb1*bb] = C1[a]^+ O_us C2[bb]   (column-major nb1 x nb2, c128)          */
+int jdft_overlap_us(const jdft_basis *b, const double *P, int nproj, const double *Q, int Q_mode, const double *C1,
+                    int nb1, const double *C2, int nb2, double *M, jdft_stream s);
 
 /* ---- the steps next to H C in an SCF / minimiser iteration (PAPER.md:127 ElecVars:
  * wavefunctions -> density -> potential; PAPER.md:76 integrals as dot products) ------------------------------ */

@@ -19,7 +19,7 @@ EXPORTS = [
     "jdft_basis_create", "jdft_basis_destroy", "jdft_basis_info", "jdft_basis_structure", "jdft_basis_export",
     "jdft_basis_device_maps", "jdft_workspace_bytes", "jdft_set_workspace", "jdft_set_option",
     "jdft_apply_I", "jdft_apply_Idag", "jdft_apply_J", "jdft_apply_L", "jdft_apply_O", "jdft_apply_Vnl",
-    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_apply_H_host", "jdft_overlap_host",
+    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_apply_H_host", "jdft_overlap_host",
     "jdft_last_error", "jdft_launch_count", "jdft_profile_read", "jdft_version",
 ]
 
@@ -53,6 +53,8 @@ def _load():
     L.jdft_apply_H.argtypes = [vp, vp, vp, ci, vp, ci, vp, ci, vp, vp]
     L.jdft_overlap.argtypes = [vp, vp, ci, vp, ci, vp, vp]
     L.jdft_subspace.argtypes = [vp, vp, ci, vp, ci, vp, vp]
+    L.jdft_apply_O_us.argtypes = [vp, vp, ci, vp, ci, vp, ci, vp, vp]
+    L.jdft_overlap_us.argtypes = [vp, vp, ci, vp, ci, vp, ci, vp, ci, vp, vp]
     L.jdft_density.argtypes = [vp, vp, ci, vp, vp, ci, vp]
     L.jdft_gradient.argtypes = [vp, vp, ci, vp, vp]
     L.jdft_divergence.argtypes = [vp, vp, ci, vp, vp]
@@ -220,6 +222,11 @@ def _PD(P, D, basis):
         if D.shape[0] != nproj:
             raise ValueError("diagonal D must have nproj entries")
         return _dev(P, torch.complex128, "P"), nproj, _dev(D, torch.float64, "D"), 0
+    if D.dim() == 3:  # per-atom Hermitian blocks [nproj / nblk, nblk, nblk]: D_mode = nblk
+        nblk = int(D.shape[1])
+        if nblk < 2 or D.shape[2] != nblk or D.shape[0] * nblk != nproj:
+            raise ValueError("block D must be [nproj / nblk, nblk, nblk] with nblk >= 2")
+        return _dev(P, torch.complex128, "P"), nproj, _dev(D, torch.complex128, "D"), nblk
     if tuple(D.shape) != (nproj, nproj):
         raise ValueError("dense D must be [nproj, nproj]")
     return _dev(P, torch.complex128, "P"), nproj, _dev(D, torch.complex128, "D"), 1
@@ -265,6 +272,28 @@ def jdft_overlap(basis, C1, C2, M=None):
         M = torch.empty((nb2, nb1), dtype=torch.complex128, device=C1.device)  # column-major nb1 x nb2
     _chk(_lib.jdft_overlap(basis._h, _dev(C1, torch.complex128, "C1"), nb1, _dev(C2, torch.complex128, "C2"), nb2,
                            _dev(M, torch.complex128, "M"), _stream()))
+    return M.t()
+
+
+def jdft_apply_O_us(basis, P, Q, C, OC=None):
+    """Ultrasoft generalised overlap operator Omega (C + P Q P^+ C); Q: [np] real, [np, np] or [np / nblk, nblk, nblk]."""
+    nb = _bands(C, basis, "C")
+    if OC is None:
+        OC = torch.empty_like(C)
+    Pp, nproj, Qp, mode = _PD(P, Q, basis)
+    _chk(_lib.jdft_apply_O_us(basis._h, Pp, nproj, Qp, mode, _dev(C, torch.complex128, "C"), nb,
+                              _dev(OC, torch.complex128, "OC"), _stream()))
+    return OC
+
+
+def jdft_overlap_us(basis, P, Q, C1, C2, M=None):
+    """M[a, b] = C1[a]^+ O_us C2[b], O_us = Omega (1 + P Q P^+) (a view of the column-major result)."""
+    nb1, nb2 = _bands(C1, basis, "C1"), _bands(C2, basis, "C2")
+    if M is None:
+        M = torch.empty((nb2, nb1), dtype=torch.complex128, device=C1.device)
+    Pp, nproj, Qp, mode = _PD(P, Q, basis)
+    _chk(_lib.jdft_overlap_us(basis._h, Pp, nproj, Qp, mode, _dev(C1, torch.complex128, "C1"), nb1,
+                              _dev(C2, torch.complex128, "C2"), nb2, _dev(M, torch.complex128, "M"), _stream()))
     return M.t()
 
 
@@ -340,7 +369,7 @@ def jdft_apply_H_host(basis, Vloc, P, D, C, HC):
         Pp, nproj, Dp, mode = None, 0, None, 0
     else:
         nproj = int(P.shape[0])
-        mode = 0 if D.dim() == 1 else 1
+        mode = 0 if D.dim() == 1 else (1 if D.dim() == 2 else int(D.shape[1]))
         Pp = _host(P, torch.complex128, "P")
         Dp = _host(D, torch.float64 if mode == 0 else torch.complex128, "D")
     _chk(_lib.jdft_apply_H_host(basis._h, _host(Vloc, torch.float64, "Vloc"), Pp, nproj, Dp, mode,

@@ -11,12 +11,33 @@ int check_ptr16(const void *p, const char *who) {
     return JDFT_OK;
 }
 
-// out (+)= P D P^+ C using the workspace for B = P^+ C, D B and the split-K partials
+// B1[ib][j] = scale * (D P^+ C)[j][ib] in the workspace; returns the array that holds it in *Bd
+//   D_mode 0: real diagonal folded into the split-K reduction; 1: dense Hermitian, a second (small) GEMM;
+//   nblk >= 2: per-atom blocks applied inside the reduction (k_splitk_reduce_block)
+int project_D(const jdft_basis *b, const double *P, int nproj, const double *D, int D_mode, const double *C, int nb,
+              double scale, double *B1, double *B2, void *part, size_t part_bytes, cudaStream_t st, const double **Bd) {
+    int rc;
+    *Bd = B1;
+    if (D_mode >= 2)
+        return jdft_gemm_dotk(b, C, nb, P, nproj, b->nG, 1, scale, nullptr, B1, part, part_bytes, st, D, D_mode);
+    if ((rc = jdft_gemm_dotk(b, C, nb, P, nproj, b->nG, 1, scale, D_mode == 0 ? D : nullptr, B1, part, part_bytes, st))) return rc;
+    if (D_mode == 1) {
+        // B2[ib][j] = sum_l D[j][l] B1[ib][l]
+        if ((rc = jdft_gemm_dotk(b, B1, nb, D, nproj, nproj, 0, 1.0, nullptr, B2, part, part_bytes, st))) return rc;
+        *Bd = B2;
+    }
+    return JDFT_OK;
+}
+
+// out (+)= scale * P D P^+ C (+ addscale * Add) using the workspace for B = P^+ C, D B and the split-K partials
 int vnl_impl(const jdft_basis *b, const double *P, int nproj, const double *D, int D_mode, const double *C, int nb,
-             double *out, int accumulate, cudaStream_t st, const char *who) {
+             double *out, int accumulate, cudaStream_t st, const char *who, double scale = 1.0,
+             const double *Add = nullptr, double addscale = 0.0) {
     if (nproj == 0 || nb == 0) {
-        if (!accumulate && nb > 0)
+        if (!accumulate && nb > 0) {
+            if (Add) return jdft_fail(JDFT_EINVAL, "%s: internal: add-source without projectors", who);
             JDFT_CUDA(cudaMemsetAsync(out, 0, (size_t)nb * b->nG * 16, st));
+        }
         return JDFT_OK;
     }
     const size_t bsz = align_up((size_t)nb * nproj * 16);
@@ -26,28 +47,23 @@ int vnl_impl(const jdft_basis *b, const double *P, int nproj, const double *D, i
     void *part = ws + 2 * bsz;
     const size_t part_bytes = b->ws_bytes - 2 * bsz;
     int rc;
-    // B1[ib][j] = D_j * sum_n conj(P[j][n]) C[ib][n]   (D folded in when diagonal)
-    if ((rc = jdft_gemm_dotk(b, C, nb, P, nproj, b->nG, 1, 1.0, D_mode == 0 ? D : nullptr, B1, part, part_bytes, st))) return rc;
-    const double *Bd = B1;
-    if (D_mode == 1) {
-        // B2[ib][j] = sum_l D[j][l] B1[ib][l]
-        if ((rc = jdft_gemm_dotk(b, B1, nb, D, nproj, nproj, 0, 1.0, nullptr, B2, part, part_bytes, st))) return rc;
-        Bd = B2;
-    }
+    const double *Bd;
+    if ((rc = project_D(b, P, nproj, D, D_mode, C, nb, scale, B1, B2, part, part_bytes, st, &Bd))) return rc;
     // out[ib][n] (+)= sum_j Bd[ib][j] P[j][n]
-    return jdft_gemm_expand(b, Bd, nb, P, nproj, b->nG, out, accumulate, st);
+    return jdft_gemm_expand(b, Bd, nb, P, nproj, b->nG, out, accumulate, st, Add, addscale);
 }
 
 int check_vnl_args(const jdft_basis *b, const double *P, int nproj, const double *D, int D_mode, const double *C, int nb,
                    const double *out, const char *who) {
     if (!b) return jdft_fail(JDFT_EINVAL, "%s: null basis", who);
     if (nb < 0 || nproj < 0) return jdft_fail(JDFT_EINVAL, "%s: negative size", who);
-    if (D_mode != 0 && D_mode != 1) return jdft_fail(JDFT_EINVAL, "%s: D_mode must be 0 or 1", who);
+    if (D_mode < 0) return jdft_fail(JDFT_EINVAL, "%s: D_mode must be 0, 1 or a block size >= 2", who);
+    if (D_mode >= 2 && nproj % D_mode != 0) return jdft_fail(JDFT_EINVAL, "%s: nproj = %d is not a multiple of the block size %d", who, nproj, D_mode);
     if (nb > 0 && (!C || !out)) return jdft_fail(JDFT_EINVAL, "%s: null data pointer", who);
     if (nproj > 0 && (!P || !D)) return jdft_fail(JDFT_EINVAL, "%s: null projector / D pointer", who);
     int rc;
     if ((rc = check_ptr16(C, who)) || (rc = check_ptr16(out, who)) || (rc = check_ptr16(P, who))) return rc;
-    if (D_mode == 1 && (rc = check_ptr16(D, who))) return rc;
+    if (D_mode >= 1 && (rc = check_ptr16(D, who))) return rc;
     return JDFT_OK;
 }
 
@@ -97,12 +113,8 @@ extern "C" int jdft_apply_H(const jdft_basis *b, const double *Vloc, const doubl
     void *part = ws + 2 * bsz;
     JDFT_CUDA(cudaEventRecord(b->ev_fork, st));
     JDFT_CUDA(cudaStreamWaitEvent(b->side, b->ev_fork, 0));
-    int rc_side = jdft_gemm_dotk(b, C, nb, P, nproj, b->nG, 1, 1.0, D_mode == 0 ? D : nullptr, B1, part, part_bytes, b->side);
-    const double *Bd = B1;
-    if (!rc_side && D_mode == 1) {
-        rc_side = jdft_gemm_dotk(b, B1, nb, D, nproj, nproj, 0, 1.0, nullptr, B2, part, part_bytes, b->side);
-        Bd = B2;
-    }
+    const double *Bd;
+    int rc_side = project_D(b, P, nproj, D, D_mode, C, nb, 1.0, B1, B2, part, part_bytes, b->side, &Bd);
     cudaEventRecord(b->ev_join, b->side);
     rc = jdft_local_H(b, Vloc, C, nb, HC, st, gemm_bytes);
     JDFT_CUDA(cudaStreamWaitEvent(st, b->ev_join, 0));  // always join, also on error
@@ -137,6 +149,47 @@ extern "C" int jdft_subspace(const jdft_basis *b, const double *C1, int nb1, con
     return jdft_gemm_dotk(b, X2, nb2, C1, nb1, b->nG, 1, 1.0, nullptr, M, b->ws, b->ws_bytes, (cudaStream_t)s);
 }
 
+// ---- ultrasoft generalised overlap (reading 24) ------------------
+// O_us C = Omega (C + P Q P^+ C): B = Omega Q P^+ C (Q folded into the split-K reduction), then ONE expand GEMM whose
+// epilogue adds Omega C, so OC is written once and C read once.
+extern "C" int jdft_apply_O_us(const jdft_basis *b, const double *P, int nproj, const double *Q, int Q_mode,
+                               const double *C, int nb, double *OC, jdft_stream s) {
+    int rc = check_vnl_args(b, P, nproj, Q, Q_mode, C, nb, OC, "apply_O_us");
+    if (rc) return rc;
+    if (nb == 0) return JDFT_OK;
+    if (nproj == 0) return jdft_apply_O(b, C, nb, OC, s);
+    return vnl_impl(b, P, nproj, Q, Q_mode, C, nb, OC, 0, (cudaStream_t)s, "apply_O_us", b->volume, C, b->volume);
+}
+
+// M = C1^+ O_us C2 = Omega C1^+ C2 + (P^+ C1)^+ (Omega Q P^+ C2): the big K = nG contraction as in jdft_overlap, the
+// projector term as two projections and one small K = nproj contraction accumulated into M by its reduction.
+extern "C" int jdft_overlap_us(const jdft_basis *b, const double *P, int nproj, const double *Q, int Q_mode,
+                               const double *C1, int nb1, const double *C2, int nb2, double *M, jdft_stream s) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "overlap_us: null basis");
+    if (nb1 < 0 || nb2 < 0) return jdft_fail(JDFT_EINVAL, "overlap_us: negative size");
+    if (nb1 == 0 || nb2 == 0) return JDFT_OK;
+    int rc = check_vnl_args(b, P, nproj, Q, Q_mode, C1, nb1, M, "overlap_us");
+    if (rc) return rc;
+    if (!C2) return jdft_fail(JDFT_EINVAL, "overlap_us: null data pointer");
+    if ((rc = check_ptr16(C2, "overlap_us"))) return rc;
+    if ((rc = jdft_overlap(b, C1, nb1, C2, nb2, M, s))) return rc;
+    if (nproj == 0) return JDFT_OK;
+    cudaStream_t st = (cudaStream_t)s;
+    const size_t bs1 = align_up((size_t)nb1 * nproj * 16), bs2 = align_up((size_t)nb2 * nproj * 16);
+    if (b->ws_bytes < bs1 + 2 * bs2 + 16 * (size_t)(nb1 > nb2 ? nb1 : nb2) * nproj)
+        return jdft_fail(JDFT_EWORKSPACE, "overlap_us: workspace too small (%zu bytes needed)", bs1 + 2 * bs2 + 16 * (size_t)(nb1 > nb2 ? nb1 : nb2) * nproj);
+    char *ws = (char *)b->ws;
+    double *A1 = (double *)ws, *B1 = (double *)(ws + bs1), *B2 = (double *)(ws + bs1 + bs2);
+    void *part = ws + bs1 + 2 * bs2;
+    const size_t part_bytes = b->ws_bytes - (bs1 + 2 * bs2);
+    // A1[a][j] = (P^+ C1)[j][a];  Bd[bb][j] = Omega (Q P^+ C2)[j][bb]
+    if ((rc = jdft_gemm_dotk(b, C1, nb1, P, nproj, b->nG, 1, 1.0, nullptr, A1, part, part_bytes, st))) return rc;
+    const double *Bd;
+    if ((rc = project_D(b, P, nproj, Q, Q_mode, C2, nb2, b->volume, B1, B2, part, part_bytes, st, &Bd))) return rc;
+    // M[bb][a] += sum_j Bd[bb][j] conj(A1[a][j])
+    return jdft_gemm_dotk(b, Bd, nb2, A1, nb1, nproj, 1, 1.0, nullptr, M, part, part_bytes, st, nullptr, 0, 1);
+}
+
 // ---- HOST-buffer variants ----------------------------------------------------------------------------------
 namespace {
 int host_buf(jdft_basis *b, int slot, size_t bytes, void **out) {
@@ -156,12 +209,12 @@ int host_buf(jdft_basis *b, int slot, size_t bytes, void **out) {
 extern "C" int jdft_apply_H_host(jdft_basis *b, const double *Vloc, const double *P, int nproj, const double *D,
                                  int D_mode, const double *C, int nb, double *HC) {
     if (!b) return jdft_fail(JDFT_EINVAL, "apply_H_host: null basis");
-    if (nb < 0 || nproj < 0 || (D_mode != 0 && D_mode != 1)) return jdft_fail(JDFT_EINVAL, "apply_H_host: bad size or mode");
+    if (nb < 0 || nproj < 0 || D_mode < 0 || (D_mode >= 2 && nproj % D_mode != 0)) return jdft_fail(JDFT_EINVAL, "apply_H_host: bad size or mode");
     if (!Vloc || (nb > 0 && (!C || !HC)) || (nproj > 0 && (!P || !D))) return jdft_fail(JDFT_EINVAL, "apply_H_host: null pointer");
     if (nb == 0) return JDFT_OK;
     JDFT_CUDA(cudaSetDevice(b->device));
     const size_t cb = (size_t)nb * b->nG * 16, vb = (size_t)b->N * 8, pb = (size_t)nproj * b->nG * 16;
-    const size_t db = D_mode == 0 ? (size_t)nproj * 8 : (size_t)nproj * nproj * 16;
+    const size_t db = D_mode == 0 ? (size_t)nproj * 8 : (D_mode == 1 ? (size_t)nproj * nproj * 16 : (size_t)nproj * D_mode * 16);
     void *dC, *dHC, *dV, *dP, *dD, *dW;
     int rc;
     if ((rc = host_buf(b, 0, cb, &dC)) || (rc = host_buf(b, 1, cb, &dHC)) || (rc = host_buf(b, 2, vb, &dV)) ||
@@ -207,13 +260,9 @@ extern "C" int jdft_apply_H_host(jdft_basis *b, const double *Vloc, const double
                     cudaError_t e2 = cudaStreamWaitEvent(st, b->ev_join, 0);
                     if (!rc && e2 != cudaSuccess) rc = jdft_cuda_fail(e2, "apply_H_host join");
                 }
-                if (!rc) rc = jdft_gemm_dotk(b, (const double *)dC, nb, (const double *)dP, nproj, b->nG, 1, 1.0,
-                                             D_mode == 0 ? (const double *)dD : nullptr, B1, ws + 2 * bsz, part_bytes, st);
                 const double *Bd = B1;
-                if (!rc && D_mode == 1) {
-                    rc = jdft_gemm_dotk(b, B1, nb, (const double *)dD, nproj, nproj, 0, 1.0, nullptr, B2, ws + 2 * bsz, part_bytes, st);
-                    Bd = B2;
-                }
+                if (!rc) rc = project_D(b, (const double *)dP, nproj, (const double *)dD, D_mode, (const double *)dC, nb, 1.0, B1, B2,
+                                        ws + 2 * bsz, part_bytes, st, &Bd);
                 if (!rc) rc = jdft_gemm_expand(b, Bd, nb, (const double *)dP, nproj, b->nG, (double *)dHC, 1, st);
             }
         }

@@ -4,7 +4,10 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
+#include <utility>
 #include "jdft_internal.h"
 
 static thread_local char g_err[512] = "";
@@ -29,6 +32,17 @@ extern "C" int64_t jdft_launch_count(int reset) {
     return v;
 }
 extern "C" const char *jdft_version(void) { return "jdft-b200 0.1 (sm_100a)"; }
+
+cudaError_t jdft_ensure_smem(const void *kernel, size_t bytes, int device) {
+    static std::mutex mu;
+    static std::map<std::pair<const void *, int>, size_t> done;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t &have = done[std::make_pair(kernel, device)];
+    if (have >= bytes && have > 0) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) have = bytes;
+    return e;
+}
 
 static bool smooth235(int n) {
     if (n < 1) return false;
@@ -124,7 +138,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     for (int i = 0; i < 8; i++) { b->hb[i] = nullptr; b->hb_bytes[i] = 0; }
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
     b->opt_profile_kernel = 0; b->prof_used = 0;
-    b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
+    b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_gemm3m = 1; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
 
     // G = 2 pi R^-1 (adjugate / det): row i of G is the reciprocal vector b_i
     {
@@ -254,6 +268,8 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
 
     // upload
     cudaError_t e = cudaSetDevice(device);
+    b->num_sms = 148;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&b->num_sms, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = upload(&b->d_index, b->index.data(), b->index.size());
     if (e == cudaSuccess) e = upload(&b->d_iG, b->iG.data(), b->iG.size());
     if (e == cudaSuccess) e = upload(&b->d_ke, b->ke.data(), b->ke.size());
@@ -336,6 +352,7 @@ extern "C" int jdft_set_option(jdft_basis *b, const char *key, int64_t value) {
     if (!strcmp(key, "band_batch")) { b->opt_band_batch = value < 0 ? 0 : value; return JDFT_OK; }
     if (!strcmp(key, "planes_pair")) { b->opt_pair = value != 0; return JDFT_OK; }
     if (!strcmp(key, "planes_prune")) { b->opt_prune = value != 0; return JDFT_OK; }
+    if (!strcmp(key, "gemm_3m")) { b->opt_gemm3m = value != 0; return JDFT_OK; }
     if (!strcmp(key, "overlap_gemm")) { b->opt_overlap = value != 0; return JDFT_OK; }
     if (!strcmp(key, "force_generic_fft")) { b->opt_force_generic = value != 0; return JDFT_OK; }
     if (!strcmp(key, "profile_kernel")) { b->opt_profile_kernel = value; b->prof_used = 0; return JDFT_OK; }

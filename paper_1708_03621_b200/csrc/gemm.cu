@@ -50,8 +50,13 @@ __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld
 
 // ---------------------------------------------------------------------------------------------- dot-K GEMM
 // BN_ = 64, or 48 when the column extent is a multiple of 48 but not of 64 (np = 288, 864: no zero-padded DMMAs)
-template <bool CONJY, bool TRI, int BN_>
-__global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
+// M3: the complex product by the 3M (Gauss) scheme -- three real DMMAs per complex tile product instead of four:
+//   k1 = (xr + xi) yr,  k2 = xr (e - yr),  k3 = xi (yr + e)   (e = +-yi),   real = k1 - k3,  imag = k1 + k2
+// (three accumulator sets; the two operand sums cost 1 + 2/MT DADD per fragment).  Normwise as accurate as the 4M
+// scheme (Higham, Accuracy and Stability, ch. 23: 3M is normwise stable), which is what the per-band relative L2
+// tolerance measures; 25 % fewer tensor instructions.
+template <bool CONJY, bool TRI, int BN_, bool M3 = false>
+__global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
                                                         const double2 *__restrict__ Y, const int Cn, const int64_t K,
                                                         const int ktiles_per_split, double2 *__restrict__ part) {
     extern __shared__ __align__(16) char smem[];
@@ -77,11 +82,15 @@ __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restric
     if (kt1 > ktiles) kt1 = ktiles;
     const int nkt = (int)(kt1 - kt0);
 
-    double cr[4][NTL][2], ci[4][NTL][2];
+    // 4M: cr = real, ci = imag accumulators.  3M: cr = k1, ci = k2, c3 = k3 accumulators.
+    double cr[4][NTL][2], ci[4][NTL][2], c3[M3 ? 4 : 1][M3 ? NTL : 1][2];
 #pragma unroll
     for (int i = 0; i < 4; i++)
 #pragma unroll
-        for (int j = 0; j < NTL; j++) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+        for (int j = 0; j < NTL; j++) {
+            cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+            if constexpr (M3) c3[i][j][0] = c3[i][j][1] = 0.0;
+        }
 
     for (int s = 0; s < STAGES - 1; s++) {
         if (s < nkt) {
@@ -113,18 +122,50 @@ __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restric
 #pragma unroll
             for (int j = 0; j < NTL; j++)
                 bq[j] = *reinterpret_cast<const double2 *>(by + kk * KBLK_BYTES + (wc + 8 * j) * 64 + fo);
+            if constexpr (M3) {
+                double sa[4], d2[NTL], s3[NTL];
 #pragma unroll
-            for (int i = 0; i < 4; i++)
+                for (int i = 0; i < 4; i++) sa[i] = a[i].x + a[i].y;
 #pragma unroll
                 for (int j = 0; j < NTL; j++) {
-                    // X (Yr -/+ i Yi):  conj: Cr += XrYr + XiYi, Ci += XiYr - XrYi ; else Cr += XrYr - XiYi, Ci += XiYr + XrYi
-                    const double yi = CONJY ? bq[j].y : -bq[j].y;
-                    dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
-                    dmma(ci[i][j][0], ci[i][j][1], a[i].y, bq[j].x);
-                    dmma(cr[i][j][0], cr[i][j][1], a[i].y, yi);
-                    dmma(ci[i][j][0], ci[i][j][1], a[i].x, -yi);
+                    const double e = CONJY ? -bq[j].y : bq[j].y;   // X (yr + i e)
+                    d2[j] = e - bq[j].x;
+                    s3[j] = bq[j].x + e;
                 }
+#pragma unroll
+                for (int i = 0; i < 4; i++)
+#pragma unroll
+                    for (int j = 0; j < NTL; j++) {
+                        dmma(cr[i][j][0], cr[i][j][1], sa[i], bq[j].x);
+                        dmma(ci[i][j][0], ci[i][j][1], a[i].x, d2[j]);
+                        dmma(c3[i][j][0], c3[i][j][1], a[i].y, s3[j]);
+                    }
+            } else {
+#pragma unroll
+                for (int i = 0; i < 4; i++)
+#pragma unroll
+                    for (int j = 0; j < NTL; j++) {
+                        // X (Yr -/+ i Yi):  conj: Cr += XrYr + XiYi, Ci += XiYr - XrYi ; else Cr += XrYr - XiYi, Ci += XiYr + XrYi
+                        const double yi = CONJY ? bq[j].y : -bq[j].y;
+                        dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
+                        dmma(ci[i][j][0], ci[i][j][1], a[i].y, bq[j].x);
+                        dmma(cr[i][j][0], cr[i][j][1], a[i].y, yi);
+                        dmma(ci[i][j][0], ci[i][j][1], a[i].x, -yi);
+                    }
+            }
         }
+    }
+    if constexpr (M3) {
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+#pragma unroll
+            for (int j = 0; j < NTL; j++)
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const double k1 = cr[i][j][h], k2 = ci[i][j][h], k3 = c3[i][j][h];
+                    cr[i][j][h] = k1 - k3;
+                    ci[i][j][h] = k1 + k2;
+                }
     }
     cp_async_wait<0>();
     double2 *P = part + (size_t)blockIdx.z * Rn * Cn;
@@ -145,7 +186,7 @@ __global__ void __launch_bounds__(NTHREADS) k_gemm_dotk(const double2 *__restric
 // tri: only tiles with row tile >= col tile were computed; the rest is the conjugate transpose (Hermitian result)
 __global__ void k_splitk_reduce(const double2 *__restrict__ part, const int nsplit, const int64_t total, const int Cn,
                                 const double scale, const double *__restrict__ dscale, double2 *__restrict__ Out,
-                                const int tri) {
+                                const int tri, const int accumulate) {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
         int64_t src = i;
         bool cj = false;
@@ -161,17 +202,82 @@ __global__ void k_splitk_reduce(const double2 *__restrict__ part, const int nspl
         }
         if (cj) si = -si;
         const double f = dscale ? scale * dscale[i % Cn] : scale;
-        Out[i] = make_double2(f * sr, f * si);
+        double2 o = make_double2(f * sr, f * si);
+        if (accumulate) { const double2 w = Out[i]; o.x += w.x; o.y += w.y; }
+        Out[i] = o;
+    }
+}
+
+// Block-diagonal D (per-atom Hermitian blocks c128[Cn / nblk][nblk][nblk], D_mode = nblk) applied in the reduction:
+// Out[r][a nblk + j] = scale * sum_l D[a][j][l] * (sum_s part[s][r][a nblk + l]).  One thread per (row, atom); the
+// nblk reduced values stay in registers (nblk <= NBMAX), so the partials are read once.
+template <int NBMAX>
+__global__ void k_splitk_reduce_block(const double2 *__restrict__ part, const int nsplit, const int Rn, const int Cn,
+                                      const int nblk, const double scale, const double2 *__restrict__ Dblk,
+                                      double2 *__restrict__ Out) {
+    const int natom = Cn / nblk;
+    const int64_t total = (int64_t)Rn * Cn, items = (int64_t)Rn * natom;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < items; i += (int64_t)gridDim.x * blockDim.x) {
+        const int r = (int)(i / natom), a = (int)(i % natom);
+        const size_t base = (size_t)r * Cn + (size_t)a * nblk;
+        double2 red[NBMAX];
+#pragma unroll
+        for (int l = 0; l < NBMAX; l++) {
+            red[l] = make_double2(0.0, 0.0);
+            if (l < nblk)
+                for (int s = 0; s < nsplit; s++) {
+                    const double2 v = part[(size_t)s * total + base + l];
+                    red[l].x += v.x;
+                    red[l].y += v.y;
+                }
+        }
+        const double2 *Da = Dblk + (size_t)a * nblk * nblk;
+        for (int j = 0; j < nblk; j++) {
+            double sr = 0.0, si = 0.0;
+#pragma unroll
+            for (int l = 0; l < NBMAX; l++)
+                if (l < nblk) {
+                    const double2 d = Da[j * nblk + l];
+                    sr += d.x * red[l].x - d.y * red[l].y;
+                    si += d.x * red[l].y + d.y * red[l].x;
+                }
+            Out[base + j] = make_double2(scale * sr, scale * si);
+        }
+    }
+}
+// any block size: one thread per output element, the block row re-reduced per element (blocks > 16 are rare)
+__global__ void k_splitk_reduce_block_any(const double2 *__restrict__ part, const int nsplit, const int Rn, const int Cn,
+                                          const int nblk, const double scale, const double2 *__restrict__ Dblk,
+                                          double2 *__restrict__ Out) {
+    const int64_t total = (int64_t)Rn * Cn;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int c = (int)(i % Cn), a = c / nblk, j = c % nblk;
+        const size_t base = (size_t)(i - c) + (size_t)a * nblk;
+        const double2 *Da = Dblk + ((size_t)a * nblk + j) * nblk;
+        double sr = 0.0, si = 0.0;
+        for (int l = 0; l < nblk; l++) {
+            double rr = 0.0, ri = 0.0;
+            for (int s = 0; s < nsplit; s++) {
+                const double2 v = part[(size_t)s * total + base + l];
+                rr += v.x;
+                ri += v.y;
+            }
+            const double2 d = Da[l];
+            sr += d.x * rr - d.y * ri;
+            si += d.x * ri + d.y * rr;
+        }
+        Out[i] = make_double2(scale * sr, scale * si);
     }
 }
 
 // ---------------------------------------------------------------------------------------------- expand GEMM
 // BN_ x (WM x WN warps): 64 x (2 x 2) is the default tile; 56 x (4 x 1) exists because for some n extents it fills the
 // 148 x 3 CTA slots in whole waves where 64 leaves a half-empty tail wave (config 2: 1.68 -> 1.93 waves).
-template <int BN_, int WM, int WN>
-__global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__restrict__ A, const int Rn,
+template <int BN_, int WM, int WN, bool M3 = false>
+__global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const double2 *__restrict__ A, const int Rn,
                                                           const double2 *__restrict__ Pm, const int K, const int64_t Nn,
-                                                          double2 *__restrict__ Out, const int accumulate) {
+                                                          double2 *Out, const double2 *Add,
+                                                          const double addscale) {
     extern __shared__ __align__(16) char smem[];
     constexpr int MTL = BM / (8 * WM), NTL = BN_ / (8 * WN);   // 8 x 8 DMMA tiles per warp along rows / columns
     constexpr int PROW = BN_ * 16 + 32, OPN = BK * PROW;
@@ -183,11 +289,14 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__re
     const int64_t n0 = (int64_t)blockIdx.x * BN_;
     const int nkt = (K + BK - 1) / BK;
 
-    double cr[MTL][NTL][2], ci[MTL][NTL][2];
+    double cr[MTL][NTL][2], ci[MTL][NTL][2], c3[M3 ? MTL : 1][M3 ? NTL : 1][2];   // 3M: k1, k2, k3 (see k_gemm_dotk)
 #pragma unroll
     for (int i = 0; i < MTL; i++)
 #pragma unroll
-        for (int j = 0; j < NTL; j++) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+        for (int j = 0; j < NTL; j++) {
+            cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+            if constexpr (M3) c3[i][j][0] = c3[i][j][1] = 0.0;
+        }
 
     auto load_p = [&](char *dst, int k0) {
 #pragma unroll
@@ -231,18 +340,49 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__re
 #pragma unroll
             for (int j = 0; j < NTL; j++)
                 bq[j] = *reinterpret_cast<const double2 *>(bp + kk * 4 * PROW + (wc + 8 * j) * 16 + fp);
+            if constexpr (M3) {
+                double sa[MTL], d2[NTL], s3[NTL];
 #pragma unroll
-            for (int i = 0; i < MTL; i++)
+                for (int i = 0; i < MTL; i++) sa[i] = a[i].x + a[i].y;
 #pragma unroll
                 for (int j = 0; j < NTL; j++) {
-                    dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
-                    dmma(ci[i][j][0], ci[i][j][1], a[i].y, bq[j].x);
-                    dmma(cr[i][j][0], cr[i][j][1], a[i].y, -bq[j].y);
-                    dmma(ci[i][j][0], ci[i][j][1], a[i].x, bq[j].y);
+                    d2[j] = bq[j].y - bq[j].x;
+                    s3[j] = bq[j].x + bq[j].y;
                 }
+#pragma unroll
+                for (int i = 0; i < MTL; i++)
+#pragma unroll
+                    for (int j = 0; j < NTL; j++) {
+                        dmma(cr[i][j][0], cr[i][j][1], sa[i], bq[j].x);
+                        dmma(ci[i][j][0], ci[i][j][1], a[i].x, d2[j]);
+                        dmma(c3[i][j][0], c3[i][j][1], a[i].y, s3[j]);
+                    }
+            } else {
+#pragma unroll
+                for (int i = 0; i < MTL; i++)
+#pragma unroll
+                    for (int j = 0; j < NTL; j++) {
+                        dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
+                        dmma(ci[i][j][0], ci[i][j][1], a[i].y, bq[j].x);
+                        dmma(cr[i][j][0], cr[i][j][1], a[i].y, -bq[j].y);
+                        dmma(ci[i][j][0], ci[i][j][1], a[i].x, bq[j].y);
+                    }
+            }
         }
     }
     cp_async_wait<0>();
+    if constexpr (M3) {
+#pragma unroll
+        for (int i = 0; i < MTL; i++)
+#pragma unroll
+            for (int j = 0; j < NTL; j++)
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const double k1 = cr[i][j][h], k2 = ci[i][j][h], k3 = c3[i][j][h];
+                    cr[i][j][h] = k1 - k3;
+                    ci[i][j][h] = k1 + k2;
+                }
+    }
 #pragma unroll
     for (int i = 0; i < MTL; i++) {
         const int r = row0 + wr + 8 * i + (lane >> 2);
@@ -251,14 +391,15 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__re
         for (int j = 0; j < NTL; j++) {
             const int64_t n = n0 + wc + 8 * j + 2 * (lane & 3);
             double2 *o = Out + (size_t)r * Nn + n;
+            const double2 *ad = Add + (size_t)r * Nn + n;   // Add may alias Out (accumulate): each element is read, then written, by this thread only
             if (n < Nn) {
                 double2 v = make_double2(cr[i][j][0], ci[i][j][0]);
-                if (accumulate) { const double2 w = o[0]; v.x += w.x; v.y += w.y; }
+                if (Add) { const double2 w = ad[0]; v.x = fma(addscale, w.x, v.x); v.y = fma(addscale, w.y, v.y); }
                 o[0] = v;
             }
             if (n + 1 < Nn) {
                 double2 v = make_double2(cr[i][j][1], ci[i][j][1]);
-                if (accumulate) { const double2 w = o[1]; v.x += w.x; v.y += w.y; }
+                if (Add) { const double2 w = ad[1]; v.x = fma(addscale, w.x, v.x); v.y = fma(addscale, w.y, v.y); }
                 o[1] = v;
             }
         }
@@ -266,29 +407,35 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_gemm_expand(const double2 *__re
 }
 
 template <class K>
-cudaError_t ensure_smem(K kernel, size_t bytes) {
-    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+cudaError_t ensure_smem(K kernel, size_t bytes, int device) {
+    return jdft_ensure_smem((const void *)kernel, bytes, device);
 }
 
 }  // namespace
 
 int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y, int Cn, int64_t K, int conjY,
                    double scale, const double *dscale, double *Out, void *scratch, size_t scratch_bytes,
-                   cudaStream_t st) {
+                   cudaStream_t st, const double *dblock, int nblk, int accumulate) {
     if (Rn <= 0 || Cn <= 0) return JDFT_OK;
+    if (dblock && (nblk < 1 || Cn % nblk != 0 || dscale || accumulate))
+        return jdft_fail(JDFT_EINVAL, "gemm: block-diagonal D needs nproj %% block == 0");
     const int64_t ktiles = (K + BK - 1) / BK;
     // X^+ X is Hermitian: compute the lower-triangle tiles only and mirror them in the reduction
-    const int tri = (X == Y && Rn == Cn && conjY && !dscale && BM == BN) ? 1 : 0;
+    const int tri = (X == Y && Rn == Cn && conjY && !dscale && !dblock && BM == BN) ? 1 : 0;
     const int trow = (Rn + BM - 1) / BM;
     // column tile: 48 instead of 64 when that removes a noticeable share of zero padding (np = 288: 320 -> 288 columns)
     const int pad64 = ((Cn + 63) / 64) * 64, pad48 = ((Cn + 47) / 48) * 48;
-    const int bn = (!tri && Cn > 64 && pad48 * 100 < pad64 * 93) ? 48 : 64;  // measured: pays at 10 % padding (np = 288), not at 3.6 % (np = 864)
+    int bn = (!tri && Cn > 64 && pad48 * 100 < pad64 * 93) ? 48 : 64;  // measured: pays at 10 % padding (np = 288), not at 3.6 % (np = 864)
+    // 3M scheme (three DMMAs per complex tile product; 64 x 48 tiles, its three accumulator sets leave no room for
+    // 64 x 64): taken when 0.8 x its padded width beats the 4M choice and K is long enough to matter
+    const bool m3 = !tri && b->opt_gemm3m && K >= 512 && pad48 * 80 < (bn == 48 ? pad48 : pad64) * 100;
+    if (m3) bn = 48;
     const int tcol = (Cn + bn - 1) / bn;
     const int tiles = tri ? trow * (trow + 1) / 2 : trow * tcol;
     const size_t one = (size_t)Rn * Cn * 16;
-    // Split K so that the grid fills whole waves of the 148 SMs x 2 resident CTAs (184 registers x 128 threads):
+    // Split K so that the grid fills whole waves of the SMs x 2 resident CTAs (184 registers x 128 threads):
     // among 1..6 waves take the smallest count whose fill tiles*nsplit / (waves*slots) is within 2 % of the best (stop at 97 %).
-    const int64_t slots = 148 * 2;
+    const int64_t slots = (int64_t)b->num_sms * 2;
     const int64_t max_by_k = ktiles / 16 > 0 ? ktiles / 16 : 1;              // at least 16 k-tiles (128 k) per slice
     const int64_t max_by_ws = (int64_t)(scratch_bytes / one);
     if (max_by_ws < 1) return jdft_fail(JDFT_EWORKSPACE, "gemm: workspace too small for a %d x %d result", Rn, Cn);
@@ -312,13 +459,15 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     const size_t smem = 2 * STAGES * OPK_BYTES;
     dim3 grid(tri ? tiles : tcol, tri ? 1 : trow, (unsigned)nsplit);
     jdft_prof_begin(b, JDFT_K_GEMM_DOTK, st);
-#define JDFT_DOTK_LAUNCH(CJ, TR, BNX)                                                                          \
+#define JDFT_DOTK_LAUNCH(...)                                                                                  \
     do {                                                                                                        \
-        JDFT_CUDA(ensure_smem(k_gemm_dotk<CJ, TR, BNX>, smem));                                                 \
-        k_gemm_dotk<CJ, TR, BNX><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, \
+        JDFT_CUDA(ensure_smem(k_gemm_dotk<__VA_ARGS__>, smem, b->device));                                      \
+        k_gemm_dotk<__VA_ARGS__><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, \
                                                                (int)per, (double2 *)scratch);                  \
     } while (0)
     if (tri) JDFT_DOTK_LAUNCH(true, true, 64);
+    else if (m3 && conjY) JDFT_DOTK_LAUNCH(true, false, 48, true);
+    else if (m3) JDFT_DOTK_LAUNCH(false, false, 48, true);
     else if (conjY && bn == 48) JDFT_DOTK_LAUNCH(true, false, 48);
     else if (conjY) JDFT_DOTK_LAUNCH(true, false, 64);
     else if (bn == 48) JDFT_DOTK_LAUNCH(false, false, 48);
@@ -328,36 +477,57 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     JDFT_LAUNCH_CHECK("k_gemm_dotk");
     const int64_t total = (int64_t)Rn * Cn;
     int64_t blocks = (total + 255) / 256;
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > b->num_sms * 8) blocks = b->num_sms * 8;
     jdft_prof_begin(b, JDFT_K_REDUCE, st);
-    k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, total, Cn, scale, dscale, (double2 *)Out, tri);
+    if (dblock) {
+        const int64_t items = (int64_t)Rn * (Cn / nblk);
+        int64_t bl = (items + 127) / 128;
+        if (bl > b->num_sms * 8) bl = b->num_sms * 8;
+        if (nblk <= 4)
+            k_splitk_reduce_block<4><<<(int)bl, 128, 0, st>>>((const double2 *)scratch, (int)nsplit, Rn, Cn, nblk, scale, (const double2 *)dblock, (double2 *)Out);
+        else if (nblk <= 9)
+            k_splitk_reduce_block<9><<<(int)bl, 128, 0, st>>>((const double2 *)scratch, (int)nsplit, Rn, Cn, nblk, scale, (const double2 *)dblock, (double2 *)Out);
+        else if (nblk <= 16)
+            k_splitk_reduce_block<16><<<(int)bl, 128, 0, st>>>((const double2 *)scratch, (int)nsplit, Rn, Cn, nblk, scale, (const double2 *)dblock, (double2 *)Out);
+        else
+            k_splitk_reduce_block_any<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, Rn, Cn, nblk, scale, (const double2 *)dblock, (double2 *)Out);
+    } else {
+        k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, total, Cn, scale, dscale, (double2 *)Out, tri, accumulate);
+    }
     jdft_prof_end(b, JDFT_K_REDUCE, st);
     JDFT_LAUNCH_CHECK("k_splitk_reduce");
     return JDFT_OK;
 }
 
 int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
-                     cudaStream_t st) {
+                     cudaStream_t st, const double *Add, double addscale) {
     if (Rn <= 0 || Nn <= 0) return JDFT_OK;
-    // tile width: 64, unless 56 fills the 148 x 3 CTA slots in whole waves noticeably better
-    const int64_t slots = 148 * 3, rt = (Rn + BM - 1) / BM;
+    if (accumulate) { Add = Out; addscale = 1.0; }   // Out += result; otherwise Out = result (+ addscale * Add)
+    // tile width: 64, unless 56 fills the SMs x 3 CTA slots in whole waves noticeably better
+    const int64_t slots = (int64_t)b->num_sms * 3, rt = (Rn + BM - 1) / BM;
     auto fill = [&](int bn) {
         const int64_t ctas = ((Nn + bn - 1) / bn) * rt, waves = (ctas + slots - 1) / slots;
         return (double)ctas / (double)(waves * slots);
     };
     const bool narrow = fill(56) > fill(64) + 0.05;
     jdft_prof_begin(b, JDFT_K_GEMM_EXPAND, st);
-    if (narrow) {
+    if (b->opt_gemm3m && K >= 64) {   // 3M scheme: 64 x 48 tiles, 2 CTAs per SM (see k_gemm_dotk)
+        constexpr int BNX = 48;
+        const size_t smem = STAGES * (OPK_BYTES + BK * (BNX * 16 + 32));
+        JDFT_CUDA(ensure_smem(k_gemm_expand<BNX, 2, 2, true>, smem, b->device));
+        dim3 grid((unsigned)((Nn + BNX - 1) / BNX), (unsigned)rt);
+        k_gemm_expand<BNX, 2, 2, true><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, (const double2 *)Add, addscale);
+    } else if (narrow) {
         constexpr int BNX = 56;
         const size_t smem = STAGES * (OPK_BYTES + BK * (BNX * 16 + 32));
-        JDFT_CUDA(ensure_smem(k_gemm_expand<BNX, 4, 1>, smem));
+        JDFT_CUDA(ensure_smem(k_gemm_expand<BNX, 4, 1>, smem, b->device));
         dim3 grid((unsigned)((Nn + BNX - 1) / BNX), (unsigned)rt);
-        k_gemm_expand<BNX, 4, 1><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, accumulate);
+        k_gemm_expand<BNX, 4, 1><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, (const double2 *)Add, addscale);
     } else {
         const size_t smem = STAGES * (OPK_BYTES + OPN_BYTES);
-        JDFT_CUDA(ensure_smem(k_gemm_expand<BN, 2, 2>, smem));
+        JDFT_CUDA(ensure_smem(k_gemm_expand<BN, 2, 2>, smem, b->device));
         dim3 grid((unsigned)((Nn + BN - 1) / BN), (unsigned)rt);
-        k_gemm_expand<BN, 2, 2><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, accumulate);
+        k_gemm_expand<BN, 2, 2><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, (const double2 *)Add, addscale);
     }
     jdft_prof_end(b, JDFT_K_GEMM_EXPAND, st);
     JDFT_LAUNCH_CHECK("k_gemm_expand");

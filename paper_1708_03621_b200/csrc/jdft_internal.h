@@ -21,6 +21,7 @@ struct jdft_basis {
     int S[3];
     int64_t N, nG;
     int device;
+    int num_sms;                              // multiProcessorCount of `device`, queried once at create
     // host copies of the sphere
     std::vector<int32_t> iG, index;
     std::vector<double> ke;
@@ -46,6 +47,7 @@ struct jdft_basis {
     // runs on the caller's stream
     int64_t opt_overlap;
     int64_t opt_pair;                         // K3 with two pencils per thread where available ("planes_pair")
+    int64_t opt_gemm3m;                       // GEMMs by the 3M complex-product scheme ("gemm_3m", default 1)
     int64_t opt_prune;                        // K3 hybrid: radix-8 butterflies pruned to the occupied planes ("planes_prune")
     cudaStream_t side;
     cudaEvent_t ev_fork, ev_join;
@@ -80,6 +82,10 @@ void jdft_count_launch(int n);
         if (e__ != cudaSuccess) return jdft_cuda_fail(e__, name); \
     } while (0)
 
+// Opt a kernel in to `bytes` of dynamic shared memory ONCE per (kernel, device): the first launch pays the
+// cudaFuncSetAttribute, later launches only a table lookup (no driver call on the hot path).
+cudaError_t jdft_ensure_smem(const void *kernel, size_t bytes, int device);
+
 // per-band scratch of the FFT path (bytes)
 size_t jdft_fft_bytes_per_band(const jdft_basis *b);
 // bands per batch given the workspace and options; 0 if not even one fits
@@ -93,9 +99,12 @@ int jdft_local_H(const jdft_basis *b, const double *Vloc, const double *C, int n
 
 // gemm.cu
 // Out[r][c] = scale * dscale[c] * sum_k X[r][k] * (conjY ? conj(Y[c][k]) : Y[c][k]);  X [Rn][K], Y [Cn][K], Out [Rn][Cn]
+// dblock != nullptr: instead of dscale, the block-diagonal matrix c128[Cn / nblk][nblk][nblk] multiplies each row's
+// blocks, Out[r][a nblk + j] = scale sum_l dblock[a][j][l] (X Y^+)[r][a nblk + l].  accumulate: Out += (plain mode only).
 int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y, int Cn, int64_t K, int conjY,
                    double scale, const double *dscale, double *Out, void *scratch, size_t scratch_bytes,
-                   cudaStream_t st);
+                   cudaStream_t st, const double *dblock = nullptr, int nblk = 0, int accumulate = 0);
 // Out[r][n] (+)= sum_j A[r][j] * Pm[j][n];  A [Rn][K] (K contiguous), Pm [K][Nn] (n contiguous), Out [Rn][Nn]
+// accumulate == 0 and Add != nullptr: Out = addscale * Add + A Pm  (Add [Rn][Nn]; may alias Out)
 int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
-                     cudaStream_t st);
+                     cudaStream_t st, const double *Add = nullptr, double addscale = 0.0);

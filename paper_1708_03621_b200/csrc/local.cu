@@ -1021,10 +1021,10 @@ __global__ void k_diag(const int64_t nG, const int64_t total, const double f0, c
 // the 256-bit global accesses of the pair / hybrid kernels need 32-byte aligned arrays (the ABI only asks for 16)
 inline bool aligned32(const void *a, const void *b = nullptr) { return ((((uintptr_t)a) | ((uintptr_t)b)) & 31) == 0; }
 
+// (static __shared__ tables count against the 48 KB default too, hence the 40 KB threshold)
 template <class K>
-cudaError_t ensure_smem(K kernel, size_t bytes) {
-    if (bytes <= 40 * 1024) return cudaSuccess;  // static __shared__ tables count against the 48 KB default too
-    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+cudaError_t ensure_smem(K kernel, size_t bytes, int device) {
+    return bytes <= 40 * 1024 ? cudaSuccess : jdft_ensure_smem((const void *)kernel, bytes, device);
 }
 
 #define SPEC_SWITCH(L, force_generic, ...)                    \
@@ -1068,11 +1068,11 @@ int launch_cols_inv(const jdft_basis *b, const double2 *C, int nbt, double2 *W1,
     SPEC_SWITCH(L, b->opt_force_generic, {
         if constexpr (jcols::Cfg<LT>::ok) {
             using F = jcols::Cfg<LT>;
-            JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT>, F::smem));
+            JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT>, F::smem, b->device));
             dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
             jcols::k_cols_inv_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
         } else {
-            JDFT_CUDA(ensure_smem(k_cols_inv<LT>, smem));
+            JDFT_CUDA(ensure_smem(k_cols_inv<LT>, smem, b->device));
             k_cols_inv<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
         }
     });
@@ -1090,12 +1090,12 @@ int launch_cols_fwd(const jdft_basis *b, const double2 *W1, int nbt, double scal
     SPEC_SWITCH(L, b->opt_force_generic, {
         if constexpr (jcols::Cfg<LT>::ok) {
             using F = jcols::Cfg<LT>;
-            JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT>, F::smem));
+            JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT>, F::smem, b->device));
             dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
             jcols::k_cols_fwd_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
                                                                scale, kin, b->d_ke, C, out);
         } else {
-            JDFT_CUDA(ensure_smem(k_cols_fwd<LT>, smem));
+            JDFT_CUDA(ensure_smem(k_cols_fwd<LT>, smem, b->device));
             k_cols_fwd<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
                                                     scale, kin, b->d_ke, C, out);
     }
@@ -1116,7 +1116,7 @@ int launch_rows(const jdft_basis *b, int nbt, double2 *W1, double2 *W2, cudaStre
             if (b->S[2] % 2 == 0 && b->opt_pair && aligned32(W1, W2)) {
                 using C = Tuned<LT>;
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
-                JDFT_CUDA(ensure_smem(k_rows_hyb<LT, FWD>, sm2));
+                JDFT_CUDA(ensure_smem(k_rows_hyb<LT, FWD>, sm2, b->device));
                 dim3 g2((b->S[2] + C::T - 1) / C::T, b->npl, nbt);
                 k_rows_hyb<LT, FWD><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
                 jdft_prof_end(b, FWD ? JDFT_K_ROWS_FWD : JDFT_K_ROWS_INV, st);
@@ -1127,11 +1127,11 @@ int launch_rows(const jdft_basis *b, int nbt, double2 *W1, double2 *W2, cudaStre
         if constexpr (Tuned<LT>::ok) {
             using C = Tuned<LT>;
             const size_t sm2 = (size_t)L * C::T * sizeof(double2);
-            JDFT_CUDA(ensure_smem(k_rows_tuned<LT, FWD>, sm2));
+            JDFT_CUDA(ensure_smem(k_rows_tuned<LT, FWD>, sm2, b->device));
             dim3 g2((b->S[2] + C::T - 1) / C::T, b->npl, nbt);
             k_rows_tuned<LT, FWD><<<g2, C::NT, sm2, st>>>(b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
         } else {
-            JDFT_CUDA(ensure_smem(k_rows<LT, FWD>, smem));
+            JDFT_CUDA(ensure_smem(k_rows<LT, FWD>, smem, b->device));
             k_rows<LT, FWD><<<grid, kNT, smem, st>>>(b->plan[1], b->d_tw[1], b->S[2], b->npl, b->ncol, b->d_rowcol, W1, W2);
         }
     });
@@ -1159,10 +1159,10 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
                 const size_t sm2 = (size_t)Q::G * L * Q::T * sizeof(double2);
                 dim3 g2((b->S[2] + Q::T - 1) / Q::T, (b->S[1] + Q::G - 1) / Q::G, nbt);
                 if (planes_prunable<Tuned<LT>>(b, L)) {
-                    JDFT_CUDA(ensure_smem(k_planes_fused2<LT, true>, sm2));
+                    JDFT_CUDA(ensure_smem(k_planes_fused2<LT, true>, sm2, b->device));
                     k_planes_fused2<LT, true><<<g2, Q::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
                 } else {
-                    JDFT_CUDA(ensure_smem(k_planes_fused2<LT>, sm2));
+                    JDFT_CUDA(ensure_smem(k_planes_fused2<LT>, sm2, b->device));
                     k_planes_fused2<LT><<<g2, Q::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
                 }
                 jdft_prof_end(b, JDFT_K_PLANES, st);
@@ -1176,10 +1176,10 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
                 dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
                 if (MODE == 1 && planes_prunable<C>(b, L)) {
-                    JDFT_CUDA(ensure_smem(k_planes_io_hyb<LT, MODE, MODE == 1>, sm2));
+                    JDFT_CUDA(ensure_smem(k_planes_io_hyb<LT, MODE, MODE == 1>, sm2, b->device));
                     k_planes_io_hyb<LT, MODE, MODE == 1><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, psi);
                 } else {
-                    JDFT_CUDA(ensure_smem(k_planes_io_hyb<LT, MODE>, sm2));
+                    JDFT_CUDA(ensure_smem(k_planes_io_hyb<LT, MODE>, sm2, b->device));
                     k_planes_io_hyb<LT, MODE><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, psi);
                 }
                 jdft_prof_end(b, JDFT_K_PLANES, st);
@@ -1193,10 +1193,10 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
                 dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
                 if (planes_prunable<C>(b, L)) {
-                    JDFT_CUDA(ensure_smem(k_planes_fused_h<LT, true>, sm2));
+                    JDFT_CUDA(ensure_smem(k_planes_fused_h<LT, true>, sm2, b->device));
                     k_planes_fused_h<LT, true><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
                 } else {
-                    JDFT_CUDA(ensure_smem(k_planes_fused_h<LT>, sm2));
+                    JDFT_CUDA(ensure_smem(k_planes_fused_h<LT>, sm2, b->device));
                     k_planes_fused_h<LT><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
                 }
                 jdft_prof_end(b, JDFT_K_PLANES, st);
@@ -1207,11 +1207,11 @@ int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, do
         if constexpr (MODE == 0 && Tuned<LT>::ok) {
             using C = Tuned<LT>;
             const size_t sm2 = (size_t)L * C::T * sizeof(double2);
-            JDFT_CUDA(ensure_smem(k_planes_fused<LT>, sm2));
+            JDFT_CUDA(ensure_smem(k_planes_fused<LT>, sm2, b->device));
             dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1], nbt);
             k_planes_fused<LT><<<g2, C::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V);
         } else {
-            JDFT_CUDA(ensure_smem(k_planes<LT, MODE>, smem));
+            JDFT_CUDA(ensure_smem(k_planes<LT, MODE>, smem, b->device));
             k_planes<LT, MODE><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, W2, V, psi);
         }
     });
@@ -1331,11 +1331,11 @@ extern "C" int jdft_density(const jdft_basis *b, const double *C_, int nb, const
                     const size_t sm2 = (size_t)L * C::T * sizeof(double2);
                     dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1]);
                     if (planes_prunable<C>(b, L)) {
-                        JDFT_CUDA(ensure_smem(k_planes_density_hyb<LT, true>, sm2));
+                        JDFT_CUDA(ensure_smem(k_planes_density_hyb<LT, true>, sm2, b->device));
                         k_planes_density_hyb<LT, true><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof,
                                                                                      w.W2, f + b0, nbt, n, acc);
                     } else {
-                        JDFT_CUDA(ensure_smem(k_planes_density_hyb<LT>, sm2));
+                        JDFT_CUDA(ensure_smem(k_planes_density_hyb<LT>, sm2, b->device));
                         k_planes_density_hyb<LT><<<g2, Hyb<LT>::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
                                                                           f + b0, nbt, n, acc);
                     }
@@ -1346,12 +1346,12 @@ extern "C" int jdft_density(const jdft_basis *b, const double *C_, int nb, const
             } else if constexpr (Tuned<LT>::ok) {
                 using C = Tuned<LT>;
                 const size_t sm2 = (size_t)L * C::T * sizeof(double2);
-                JDFT_CUDA(ensure_smem(k_planes_density_tuned<LT>, sm2));
+                JDFT_CUDA(ensure_smem(k_planes_density_tuned<LT>, sm2, b->device));
                 dim3 g2((b->S[2] + C::T - 1) / C::T, b->S[1]);
                 k_planes_density_tuned<LT><<<g2, C::NT, sm2, st>>>(b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
                                                                    f + b0, nbt, n, acc);
             } else {
-                JDFT_CUDA(ensure_smem(k_planes_density<LT>, smem));
+                JDFT_CUDA(ensure_smem(k_planes_density<LT>, smem, b->device));
                 k_planes_density<LT><<<grid, kNT, smem, st>>>(b->plan[0], b->d_tw[0], b->S[1], b->S[2], b->npl, b->d_planeof, w.W2,
                                                               f + b0, nbt, n, acc);
             }
@@ -1369,14 +1369,14 @@ Mat3 mat3_of(const jdft_basis *b) {
     for (int i = 0; i < 3; i++) m.k[i] = b->k[i];
     return m;
 }
-int elementwise_grid(int64_t total) {
-    int64_t blocks = (total + 255) / 256;
-    return (int)(blocks > 148 * 16 ? 148 * 16 : blocks);
+int elementwise_grid(const jdft_basis *b, int64_t total) {
+    const int64_t blocks = (total + 255) / 256, cap = (int64_t)b->num_sms * 16;
+    return (int)(blocks > cap ? cap : blocks);
 }
 int launch_gradient(const jdft_basis *b, const double *C, int nb, double *out, cudaStream_t st) {
     const int64_t total = (int64_t)nb * b->nG;
     jdft_prof_begin(b, JDFT_K_DIAG, st);
-    k_gradient<<<elementwise_grid(total), 256, 0, st>>>(mat3_of(b), b->d_iG, b->nG, total, reinterpret_cast<const double2 *>(C),
+    k_gradient<<<elementwise_grid(b, total), 256, 0, st>>>(mat3_of(b), b->d_iG, b->nG, total, reinterpret_cast<const double2 *>(C),
                                                         reinterpret_cast<double2 *>(out));
     jdft_prof_end(b, JDFT_K_DIAG, st);
     JDFT_LAUNCH_CHECK("k_gradient");
@@ -1385,7 +1385,7 @@ int launch_gradient(const jdft_basis *b, const double *C, int nb, double *out, c
 int launch_divergence(const jdft_basis *b, const double *X, int nb, double f, double *out, cudaStream_t st) {
     const int64_t total = (int64_t)nb * b->nG;
     jdft_prof_begin(b, JDFT_K_DIAG, st);
-    k_divergence<<<elementwise_grid(total), 256, 0, st>>>(mat3_of(b), b->d_iG, b->nG, total, f, reinterpret_cast<const double2 *>(X),
+    k_divergence<<<elementwise_grid(b, total), 256, 0, st>>>(mat3_of(b), b->d_iG, b->nG, total, f, reinterpret_cast<const double2 *>(X),
                                                           reinterpret_cast<double2 *>(out));
     jdft_prof_end(b, JDFT_K_DIAG, st);
     JDFT_LAUNCH_CHECK("k_divergence");
@@ -1432,10 +1432,8 @@ static int diag_op(const jdft_basis *b, const double *C, int nb, double *out, do
     if (rc) return rc;
     const int64_t total = (int64_t)nb * b->nG;
     if (total == 0) return JDFT_OK;
-    int64_t blocks = (total + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
     jdft_prof_begin(b, JDFT_K_DIAG, (cudaStream_t)s);
-    k_diag<<<(int)blocks, 256, 0, (cudaStream_t)s>>>(b->nG, total, f0, f1, b->d_ke, reinterpret_cast<const double2 *>(C),
+    k_diag<<<elementwise_grid(b, total), 256, 0, (cudaStream_t)s>>>(b->nG, total, f0, f1, b->d_ke, reinterpret_cast<const double2 *>(C),
                                                       reinterpret_cast<double2 *>(out));
     jdft_prof_end(b, JDFT_K_DIAG, (cudaStream_t)s);
     JDFT_LAUNCH_CHECK(who);

@@ -87,6 +87,10 @@ def test_null_and_bad_arguments_return_status_codes_without_a_device(lib):
         assert fn(None, None, 1, None, None) == EINVAL
     lib.jdft_pcm_hessian.argtypes = [vp, vp, vp, ctypes.c_int, vp, vp]
     assert lib.jdft_pcm_hessian(None, None, None, 1, None, None) == EINVAL
+    lib.jdft_apply_O_us.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp]
+    assert lib.jdft_apply_O_us(None, None, 0, None, 0, None, 1, None, None) == EINVAL
+    lib.jdft_overlap_us.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp]
+    assert lib.jdft_overlap_us(None, None, 0, None, 0, None, 1, None, 1, None, None) == EINVAL
     lib.jdft_version.restype = ctypes.c_char_p
     assert lib.jdft_version().startswith(b"jdft-b200")
 

@@ -414,26 +414,73 @@ def test_specialised_lengths_on_every_axis(ref, jd, cfg_id):
     assert np.linalg.norm(n_got - n_want) <= TOL * np.linalg.norm(n_want)
 
 
-# ------------------------------------------------------------------------------------------ SURVEY 8(f) rank 2 (by composition)
+# ------------------------------------------------------------------------------------------ SURVEY 8(f) rank 2 (ultrasoft)
 
-def test_ultrasoft_overlap_and_dense_D_by_composition(case, jd):
-    """Generalised (ultrasoft) overlap O C = Omega (C + P Q P^+ C) and H with a dense Hermitian D need no new kernel:
-    jdft_apply_O followed by jdft_apply_Vnl(P, Omega Q, C, out, accumulate) -- checked against the oracle's operators
-    and against the defining dense matrix on the subspace: C^+ O_us C = Omega (C^+ C + B^+ Q B), B = P^+ C."""
+def _herm_blocks(rng, natoms, nblk, psd=False, scale=1.0):
+    A = rng.standard_normal((natoms, nblk, nblk)) + 1j * rng.standard_normal((natoms, nblk, nblk))
+    H = A @ A.conj().transpose(0, 2, 1) if psd else A + A.conj().transpose(0, 2, 1)
+    return np.ascontiguousarray(scale * H)
+
+
+def _nblk(case):
+    n = case.P.shape[0]
+    return 9 if n % 9 == 0 else 4
+
+
+def test_block_diagonal_D(case, jd):
+    """Per-atom Hermitian D blocks (D_mode = nblk, applied inside the split-K reduction) in apply_Vnl and apply_H
+    against the oracle; every small shape (blocks of 4 and 9 projectors), accumulate mode included."""
+    rng = np.random.default_rng(71)
+    nblk = _nblk(case)
+    Db = _herm_blocks(rng, case.P.shape[0] // nblk, nblk)
+    want = case.rb.apply_Vnl(case.P, Db, case.C)
+    got = jd.jdft_apply_Vnl(case.gb, dev(case.P), dev(Db), dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(got, want) <= TOL
+    wantH = case.rb.apply_H(case.V, case.P, Db, case.C)
+    gotH = jd.jdft_apply_H(case.gb, dev(case.V.reshape(-1)), dev(case.P), dev(Db), dev(case.C)).cpu().numpy()
+    assert rel_err_per_band(gotH, wantH) <= TOL
+    # blocks of 2 (the projector count of every small shape is even) and one block of all projectors (> 16: generic kernel)
+    for nb2 in (2, case.P.shape[0]):
+        D2 = _herm_blocks(rng, case.P.shape[0] // nb2, nb2)
+        got = jd.jdft_apply_Vnl(case.gb, dev(case.P), dev(D2), dev(case.C)).cpu().numpy()
+        assert rel_err_per_band(got, case.rb.apply_Vnl(case.P, D2, case.C)) <= TOL
+    with pytest.raises(jd.JdftError) as e:
+        jd._chk(jd._lib.jdft_apply_Vnl(case.gb._h, dev(case.P).data_ptr(), case.P.shape[0], dev(Db).data_ptr(),
+                                      case.P.shape[0] + 1, dev(case.C).data_ptr(), case.nb, dev(case.C).data_ptr(), 0, None))
+    assert e.value.code == jd.JDFT_EINVAL
+
+
+def test_ultrasoft_apply_O_us_and_overlap_us(case, jd):
+    """O_us C = Omega (C + P Q P^+ C) and M = C1^+ O_us C2 against the oracle for all three Q layouts, plus the
+    reduction to the norm-conserving O at np = 0, in-place operation, and Hermiticity / positivity of M for PSD Q."""
     rng = np.random.default_rng(101)
     n = case.P.shape[0]
+    nblk = _nblk(case)
     A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
-    Q = 0.05 * (A + A.conj().T)
-    Om = case.rb.volume
-    out = jd.jdft_apply_O(case.gb, dev(case.C))
-    jd.jdft_apply_Vnl(case.gb, dev(case.P), dev(Om * Q), dev(case.C), out, accumulate=True)
-    got = out.cpu().numpy()
-    want = case.rb.apply_O(case.C) + case.rb.apply_Vnl(case.P, Om * Q, case.C)
-    assert rel_err_per_band(got, want) <= TOL
-    B = case.P.conj() @ case.C.T                                  # [np, nb] = P^+ C with P stored [np][nG]
-    M_def = Om * (case.C.conj() @ case.C.T + B.conj().T @ Q @ B)
-    M_gpu = jd.jdft_subspace(case.gb, dev(case.C), out).cpu().numpy()
-    assert np.max(np.abs(M_gpu - M_def)) <= 1e-10 * np.max(np.abs(M_def))
+    Qs = [_herm_blocks(rng, n // nblk, nblk, psd=True, scale=0.05), 0.05 * (A + A.conj().T), rng.uniform(0.0, 0.3, n)]
+    C2 = case.C[: max(1, case.nb // 2)] + 0.1 * (rng.standard_normal((max(1, case.nb // 2), case.rb.nG)) + 0j)
+    dP, dC, dC2 = dev(case.P), dev(case.C), dev(C2)
+    for Q in Qs:
+        got = jd.jdft_apply_O_us(case.gb, dP, dev(Q), dC).cpu().numpy()
+        assert rel_err_per_band(got, case.rb.apply_O_us(case.P, Q, case.C)) <= TOL
+        M = jd.jdft_overlap_us(case.gb, dP, dev(Q), dC, dC2).cpu().numpy()
+        want = case.rb.overlap_us(case.P, Q, case.C, C2)
+        assert M.shape == want.shape
+        assert rel_err_per_band(M.T, want.T) <= TOL
+        Ms = jd.jdft_overlap_us(case.gb, dP, dev(Q), dC, dC).cpu().numpy()     # same array on both sides
+        assert rel_err_per_band(Ms.T, case.rb.overlap_us(case.P, Q, case.C, case.C).T) <= TOL
+        assert np.max(np.abs(Ms - Ms.conj().T)) <= 1e-12 * np.max(np.abs(Ms))
+    Mpsd = jd.jdft_overlap_us(case.gb, dP, dev(Qs[0]), dC, dC).cpu().numpy()
+    assert np.all(np.linalg.eigvalsh((Mpsd + Mpsd.conj().T) / 2) > 0)
+    # in place
+    buf = dC.clone()
+    jd.jdft_apply_O_us(case.gb, dP, dev(Qs[0]), buf, buf)
+    assert rel_err_per_band(buf.cpu().numpy(), case.rb.apply_O_us(case.P, Qs[0], case.C)) <= TOL
+    # no projectors: O_us = O
+    got0 = jd.jdft_apply_O_us(case.gb, None, None, dC).cpu().numpy()
+    assert rel_err_per_band(got0, case.rb.apply_O(case.C)) <= 1e-14
+    M0 = jd.jdft_overlap_us(case.gb, None, None, dC, dC2).cpu().numpy()
+    assert rel_err_per_band(M0.T, case.rb.overlap(case.C, C2).T) <= TOL
 
 
 @pytest.mark.parametrize("cfg_id", [210, 211, 212, 213, 214, 215, 216])
@@ -523,3 +570,29 @@ def test_planes_pruned_butterflies_match(ref, jd, cfg_id):
     psi0 = jd.jdft_apply_I(c.gb, dev(c.C)).cpu().numpy().reshape(c.nb, -1)
     jd.jdft_set_option(c.gb, "planes_prune", 1)
     assert rel_err_per_band(psi1, want_psi) <= TOL and rel_err_per_band(psi0, want_psi) <= TOL
+
+
+# ------------------------------------------------------------------------------------------ 3M complex GEMM scheme
+
+@pytest.mark.parametrize("cfg_id", [102, 103, 104])
+def test_gemm_3m_and_4m_schemes_match_the_oracle(ref, jd, cfg_id):
+    """The projector GEMMs run the 3M complex-product scheme by default (three DMMAs per tile product, option
+    "gemm_3m"); both schemes must meet the tolerance on the nonlocal term ALONE (where a GEMM error cannot hide behind
+    the kinetic term), on the projection, and on a distinct-operand overlap."""
+    c = Case(ref, jd, cfg_id)
+    want = c.rb.apply_Vnl(c.P, c.D, c.C)
+    wantB = c.rb.project(c.P, c.C)
+    rng = np.random.default_rng(7)
+    C2 = np.ascontiguousarray(c.C[::-1] * (1.0 + 0.5j)) + 0.1 * rng.standard_normal(c.C.shape)
+    wantM = c.rb.overlap(c.C, C2)
+    res = {}
+    for m3 in (0, 1):
+        jd.jdft_set_option(c.gb, "gemm_3m", m3)
+        got = jd.jdft_apply_Vnl(c.gb, dev(c.P), dev(c.D), dev(c.C)).cpu().numpy()
+        assert rel_err_per_band(got, want) <= TOL
+        B = jd.jdft_project(c.gb, dev(c.P), dev(c.C)).cpu().numpy()
+        assert rel_err_per_band(B, wantB) <= TOL
+        M = jd.jdft_overlap(c.gb, dev(c.C), dev(C2)).cpu().numpy()
+        assert rel_err_per_band(M.T, wantM.T) <= TOL
+        res[m3] = got
+    assert rel_err_per_band(res[0], res[1]) <= 1e-12

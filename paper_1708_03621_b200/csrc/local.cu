@@ -7,6 +7,7 @@
 //   K5 k_cols_fwd   forward FFT along axis 2 (+) gather box -> sphere (+) + Omega ke C   (the -1/2 L C term)
 // Intermediates: W1 [nbatch][ncol][S2] and W2 [nbatch][npl][S1][S2] (c128) in the caller's workspace.
 #include <cmath>
+#include <cuda.h>
 #include "fft.cuh"
 #include "cols_tuned.cuh"
 
@@ -1017,6 +1018,8 @@ __global__ void k_diag(const int64_t nG, const int64_t total, const double f0, c
     }
 }
 
+#include "planes_tma.cuh"
+
 // ------------------------------------------------------------------------------------------------ launch helpers
 // the 256-bit global accesses of the pair / hybrid kernels need 32-byte aligned arrays (the ABI only asks for 16)
 inline bool aligned32(const void *a, const void *b = nullptr) { return ((((uintptr_t)a) | ((uintptr_t)b)) & 31) == 0; }
@@ -1146,11 +1149,70 @@ bool planes_prunable(const jdft_basis *b, int L) {
     return C::R1 == 8 && b->opt_prune && b->m0lo < 0 && b->m0lo + b->npl <= 2 * C::R2 && L + b->m0lo >= 6 * C::R2;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn tensor_map_encoder() {
+    static EncodeTiledFn fn = []() -> EncodeTiledFn {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        return (EncodeTiledFn)p;
+    }();
+    return fn;
+}
+
+// K3 through TMA (planes_tma.cuh): returns 1 if launched, 0 if this shape / pointer cannot take the path, < 0 on error
+template <int LT>
+int try_planes_tma(const jdft_basis *b, int nbt, double2 *W2, const double *V, cudaStream_t st) {
+    if constexpr (!PlanesTma<LT>::ok) {
+        return 0;
+    } else {
+        using Q = PlanesTma<LT>;
+        const int S1 = b->S[1], S2 = b->S[2], npl = b->npl;
+        EncodeTiledFn enc = tensor_map_encoder();
+        const size_t smem = Q::smem_bytes(npl);
+        if (!enc || !b->opt_tma || npl > 256 || S1 > 65536 || smem > 200 * 1024 || (((uintptr_t)W2) & 15)) return 0;
+        CUtensorMap tm;
+        const cuuint64_t gdim[3] = {(cuuint64_t)2 * S2, (cuuint64_t)S1, (cuuint64_t)nbt * npl};
+        const cuuint64_t gstr[2] = {(cuuint64_t)S2 * 16, (cuuint64_t)S1 * S2 * 16};
+        const cuuint32_t box[3] = {32, 1, (cuuint32_t)npl}, estr[3] = {1, 1, 1};
+        if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, W2, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return 0;
+        const int ntx = (S2 + Q::T - 1) / Q::T;
+        const int64_t ntiles = (int64_t)ntx * S1 * nbt;
+        if (ntiles >= ((int64_t)1 << 31)) return 0;
+        const int grid = (int)(ntiles < (int64_t)b->num_sms * Q::MINB ? ntiles : (int64_t)b->num_sms * Q::MINB);
+        const bool pr = planes_prunable<Tuned<LT>>(b, LT);
+        jdft_prof_begin(b, JDFT_K_PLANES, st);
+        if (pr) {
+            JDFT_CUDA(jdft_ensure_smem((const void *)k_planes_tma<LT, true>, smem, b->device));
+            k_planes_tma<LT, true><<<grid, Q::NT, smem, st>>>(tm, b->d_tw[0], S1, S2, npl, b->d_planeof, V, ntx, (int)ntiles);
+        } else {
+            JDFT_CUDA(jdft_ensure_smem((const void *)k_planes_tma<LT, false>, smem, b->device));
+            k_planes_tma<LT, false><<<grid, Q::NT, smem, st>>>(tm, b->d_tw[0], S1, S2, npl, b->d_planeof, V, ntx, (int)ntiles);
+        }
+        jdft_prof_end(b, JDFT_K_PLANES, st);
+        JDFT_LAUNCH_CHECK("k_planes_tma");
+        return 1;
+    }
+}
+
 template <int MODE>
 int launch_planes(const jdft_basis *b, int nbt, double2 *W2, const double *V, double2 *psi, cudaStream_t st) {
     const int L = b->S[0];
     const size_t smem = 2 * (size_t)L * kT * sizeof(double2) + (size_t)L * sizeof(int);
     dim3 grid((b->S[2] + kT - 1) / kT, b->S[1], nbt);
+    if (MODE == 0 && b->opt_tma) {
+        int took = 0;
+        SPEC_SWITCH(L, b->opt_force_generic, { took = try_planes_tma<LT>(b, nbt, W2, V, st); });
+        if (took != 0) return took < 0 ? took : JDFT_OK;
+    }
     jdft_prof_begin(b, JDFT_K_PLANES, st);
     SPEC_SWITCH(L, b->opt_force_generic, {
         if constexpr (MODE == 0 && Pair<LT>::ok && LT == 72) {  // measured: +7 % at 72 (32 pencils/CTA), -12 % at 80 (16 pencils, 80 threads)

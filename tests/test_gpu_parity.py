@@ -439,8 +439,9 @@ def test_block_diagonal_D(case, jd):
     wantH = case.rb.apply_H(case.V, case.P, Db, case.C)
     gotH = jd.jdft_apply_H(case.gb, dev(case.V.reshape(-1)), dev(case.P), dev(Db), dev(case.C)).cpu().numpy()
     assert rel_err_per_band(gotH, wantH) <= TOL
-    # blocks of 2 (the projector count of every small shape is even) and one block of all projectors (> 16: generic kernel)
-    for nb2 in (2, case.P.shape[0]):
+    # the smallest block size that divides the projector count, and ONE block of all projectors (> 16: generic kernel)
+    n = case.P.shape[0]
+    for nb2 in (min(d for d in range(2, n + 1) if n % d == 0), n):
         D2 = _herm_blocks(rng, case.P.shape[0] // nb2, nb2)
         got = jd.jdft_apply_Vnl(case.gb, dev(case.P), dev(D2), dev(case.C)).cpu().numpy()
         assert rel_err_per_band(got, case.rb.apply_Vnl(case.P, D2, case.C)) <= TOL
@@ -483,12 +484,14 @@ def test_ultrasoft_apply_O_us_and_overlap_us(case, jd):
     assert rel_err_per_band(M0.T, case.rb.overlap(case.C, C2).T) <= TOL
 
 
+@pytest.mark.parametrize("tma", [0, 1])
 @pytest.mark.parametrize("cfg_id", [210, 211, 212, 213, 214, 215, 216])
-def test_planes_pair_kernel_matches(ref, jd, cfg_id):
+def test_planes_pair_kernel_matches(ref, jd, cfg_id, tma):
     """Plane length 72 runs K3 with two pencils per thread (256-bit global accesses); same result as the one-pencil
     kernel and as the oracle; lengths 128 and 80 run the hybrid (pairs in the first and last pass only; also K2/K4 at row
     length 128).  214 and 215 have an odd S2, where the 256-bit variants must step aside for the one-pencil kernels."""
     c = Case(ref, jd, cfg_id)
+    jd.jdft_set_option(c.gb, "planes_tma", tma)      # tma = 1: K3 takes the TMA kernel wherever the plane length has one
     want = c.rb.apply_H(c.V, c.P, c.D, c.C)
     args = (dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C))
     a = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
@@ -546,12 +549,14 @@ def test_band_shards_compose_on_one_gpu(case, jd, world):
     assert rel_err_per_band(HC, want_H) <= TOL
 
 
+@pytest.mark.parametrize("tma", [0, 1])
 @pytest.mark.parametrize("cfg_id", [211, 212, 217])
-def test_planes_pruned_butterflies_match(ref, jd, cfg_id):
+def test_planes_pruned_butterflies_match(ref, jd, cfg_id, tma):
     """K3 hybrid (plane lengths 80, 128): radix-8 first/last butterflies pruned to the sphere's axis-0 extent (inputs /
     outputs 2..5 are empty planes).  211 (|m0| <= 13 of 80) and 212 (|m0| <= 21 of 128) take the pruned kernel, 217
     (|m0| <= 22 of 80, planes 20..22 occupied) must fall back; all equal the unpruned kernel and the oracle."""
     c = Case(ref, jd, cfg_id)
+    jd.jdft_set_option(c.gb, "planes_tma", tma)
     m0 = c.rb.iG[:, 0]
     L, R2 = c.rb.shape[0], c.rb.shape[0] // 8
     assert (max(m0.max(), -m0.min()) < 2 * R2) == (cfg_id != 217)
@@ -596,3 +601,37 @@ def test_gemm_3m_and_4m_schemes_match_the_oracle(ref, jd, cfg_id):
         assert rel_err_per_band(M.T, wantM.T) <= TOL
         res[m3] = got
     assert rel_err_per_band(res[0], res[1]) <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------ K3 through TMA
+
+@pytest.mark.parametrize("cfg_id", [104, 210, 211, 212, 214, 215, 217, 204, 1])
+def test_planes_tma_kernel_matches(ref, jd, cfg_id):
+    """K3 with tensor-map (TMA) loads / stores and persistent double-buffered CTAs (plane lengths 64, 72, 80, 96, 120, 128)
+    against the LSU kernels and the oracle: ragged last i2 tile (S2 = 27, 25, 50: zero-filled on load, clipped on
+    store), odd S2, pruned and unpruned butterflies, several band batches (more tiles than resident CTAs or fewer),
+    and a workspace that is only 16-byte aligned."""
+    c = Case(ref, jd, cfg_id)
+    want = c.rb.apply_H(c.V, c.P, c.D, c.C)
+    args = (dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C))
+    out = {}
+    for tma in (1, 0):
+        jd.jdft_set_option(c.gb, "planes_tma", tma)
+        out[tma] = jd.jdft_apply_H(c.gb, *args).cpu().numpy()
+        assert rel_err_per_band(out[tma], want) <= TOL
+    assert rel_err_per_band(out[1], out[0]) <= 1e-13
+    jd.jdft_set_option(c.gb, "planes_tma", 1)
+    for batch in (1, 2):
+        jd.jdft_set_option(c.gb, "band_batch", batch)
+        assert rel_err_per_band(jd.jdft_apply_H(c.gb, *args).cpu().numpy(), out[1]) <= 1e-13
+    jd.jdft_set_option(c.gb, "band_batch", 0)
+    ws = torch.empty(jd.jdft_workspace_bytes(c.gb, c.nb, max(c.nb, c.P.shape[0])) + 64, dtype=torch.uint8, device="cuda")
+    jd.jdft_set_workspace(c.gb, ws[16:])
+    assert rel_err_per_band(jd.jdft_apply_H(c.gb, *args).cpu().numpy(), want) <= TOL
+    # Listing 1 rides the same pipeline (epsilon in place of V_loc, 3 nb components)
+    rng = np.random.default_rng(5)
+    eps = 1.0 + 78.0 * rng.random(c.rb.shape)
+    phi = c.C[:2]
+    jd.jdft_set_workspace(c.gb, torch.empty(jd.jdft_workspace_bytes(c.gb, 6, 0) + 48 * 2 * c.gb.nG + 4096, dtype=torch.uint8, device="cuda"))
+    got = jd.jdft_pcm_hessian(c.gb, dev(eps.reshape(-1)), dev(phi)).cpu().numpy()
+    assert rel_err_per_band(got, c.rb.pcm_hessian(eps, phi)) <= TOL

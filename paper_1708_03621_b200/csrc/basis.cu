@@ -138,7 +138,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     for (int i = 0; i < 8; i++) { b->hb[i] = nullptr; b->hb_bytes[i] = 0; }
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
     b->opt_profile_kernel = 0; b->prof_used = 0;
-    b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_gemm3m = 1; b->opt_tma = 1; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
+    b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_gemm3m = 1; b->opt_tma = 0; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
 
     // G = 2 pi R^-1 (adjugate / det): row i of G is the reciprocal vector b_i
     {
@@ -200,6 +200,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     for (int64_t n = 0; n < b->nG; n++)
         b->index[n] = (wrap(b->iG[3 * n], S[0]) * S[1] + wrap(b->iG[3 * n + 1], S[1])) * S[2] + wrap(b->iG[3 * n + 2], S[2]);
 
+    for (int d = 0; d < 3; d++) { b->mmin[d] = mn[d]; b->mmax[d] = mx[d]; }
     // plane / column tables
     b->m0lo = mn[0];
     b->npl = mx[0] - mn[0] + 1;

@@ -90,7 +90,23 @@ __device__ __forceinline__ void mid_pass_inplace(double2 *X, const double2 *__re
 }
 
 // ------------------------------------------------------------------------------------------------ K1
-template <int LT>
+// PR (radix-8 first pass only): every column's sphere run lies in rows [0, 2 NB0) u [6 NB0, L) (|m2| < 2 NB0, true for
+// the cubic workloads of BASELINE.json), so inputs 2..5 of every first-pass butterfly are zero: they are neither read
+// nor tested, and the butterfly is the pruned dft8_in0167 (16 instead of 24 complex additions).
+template <int SIGN>
+__device__ __forceinline__ void dft8_in0167_c(double2 (&a)[8]) {
+    const double2 j6 = mul_i<SIGN>(a[6]);
+    const double2 e0 = cadd(a[0], a[6]), e2 = csub(a[0], a[6]), e1 = csub(a[0], j6), e3 = cadd(a[0], j6);
+    const double2 u = mul_w<SIGN, 1, 8>(a[1]), v = mul_w<SIGN, 7, 8>(a[7]);
+    const double2 o0 = cadd(a[1], a[7]), o2 = mul_i<SIGN>(csub(a[1], a[7]));
+    const double2 o1 = cadd(u, v), o3 = mul_i<SIGN>(csub(u, v));
+    a[0] = cadd(e0, o0); a[4] = csub(e0, o0);
+    a[1] = cadd(e1, o1); a[5] = csub(e1, o1);
+    a[2] = cadd(e2, o2); a[6] = csub(e2, o2);
+    a[3] = cadd(e3, o3); a[7] = csub(e3, o3);
+}
+
+template <int LT, bool PR = false>
 __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tuned(const double2 *__restrict__ tw, const int ncol,
                                                                 const int64_t nG, const int *__restrict__ col_n0,
                                                                 const int *__restrict__ col_m2lo,
@@ -130,6 +146,7 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tun
                 const int m2w = s_m2w[t], len = t < nc ? s_n0[t + 1] - s_n0[t] : 0;
 #pragma unroll
                 for (int k = 0; k < R0; k++) {
+                    if (PR && k >= 2 && k < 6) continue;
                     const int row = bf + k * NB0;
                     int off = row - m2w;
                     if (off < 0) off += L;
@@ -142,7 +159,8 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tun
             for (int r = 0; r < RD; r++) {
                 const int w = tid + r * NT;
                 const int t = w % T, bf = w / T;
-                Dft<R0, +1>::run(a[r]);
+                if constexpr (PR && R0 == 8) dft8_in0167_c<+1>(a[r]);
+                else Dft<R0, +1>::run(a[r]);
                 tw_mul<R0, +1>(a[r], tw, bf);
 #pragma unroll
                 for (int j = 0; j < R0; j++) X[F::sw(bf * R0 + j, t)] = a[r][j];

@@ -55,23 +55,29 @@ __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld
 // (three accumulator sets; the two operand sums cost 1 + 2/MT DADD per fragment).  Normwise as accurate as the 4M
 // scheme (Higham, Accuracy and Stability, ch. 23: 3M is normwise stable), which is what the per-band relative L2
 // tolerance measures; 25 % fewer tensor instructions.
-template <bool CONJY, bool TRI, int BN_, bool M3 = false>
+template <bool CONJY, bool TRI, int BN_, bool M3 = false, int ST = STAGES>
 __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
                                                         const double2 *__restrict__ Y, const int Cn, const int64_t K,
                                                         const int ktiles_per_split, double2 *__restrict__ part) {
     extern __shared__ __align__(16) char smem[];
-    char *sX = smem, *sY = smem + STAGES * OPK_BYTES;
+    char *sX = smem, *sY = smem + ST * OPK_BYTES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NTL = BN_ / 16;   // 8-wide DMMA tiles per warp along the columns
     const int wr = (warp >> 1) * 32, wc = (warp & 1) * (BN_ / 2);
-    // tri: X == Y and the result is Hermitian; blockIdx.x enumerates the lower-triangle tiles (row tile >= col tile)
+    // tri: X == Y and the result is Hermitian; blockIdx.x enumerates, row tile by row tile, the tiles that reach the
+    // diagonal or lie below it (first column of the tile <= last row of the tile); the reduction mirrors the rest
     int tr = blockIdx.y, tc = blockIdx.x;
     if constexpr (TRI) {
-        const int t = blockIdx.x;
-        tr = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
-        while ((tr + 1) * (tr + 2) / 2 <= t) tr++;
-        while (tr * (tr + 1) / 2 > t) tr--;
-        tc = t - tr * (tr + 1) / 2;
+        const int tcol = (Cn + BN_ - 1) / BN_;
+        int t = blockIdx.x;
+        tr = 0;
+        for (;;) {
+            const int nt = min(tcol, ((tr + 1) * BM - 1) / BN_ + 1);
+            if (t < nt) break;
+            t -= nt;
+            tr++;
+        }
+        tc = t;
     }
     const int row0 = tr * BM, col0 = tc * BN_;
     // rows of Y this tile owns (the loader fills the rest of its 64 rows with zeros); 64: exactly the original code path
@@ -92,7 +98,7 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
             if constexpr (M3) c3[i][j][0] = c3[i][j][1] = 0.0;
         }
 
-    for (int s = 0; s < STAGES - 1; s++) {
+    for (int s = 0; s < ST - 1; s++) {
         if (s < nkt) {
             load_opk(sX + s * OPK_BYTES, X, K, Rn, row0, (kt0 + s) * BK, K, tid);
             load_opk(sY + s * OPK_BYTES, Y, K, cend, col0, (kt0 + s) * BK, K, tid);
@@ -101,18 +107,18 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
     }
     const int fo = (lane >> 2) * 64 + (lane & 3) * 16;  // fragment offset inside a [64][4] block
     for (int kt = 0; kt < nkt; kt++) {
-        cp_async_wait<STAGES - 2>();
+        cp_async_wait<ST - 2>();
         __syncthreads();
         {
-            const int nx = kt + STAGES - 1;
+            const int nx = kt + ST - 1;
             if (nx < nkt) {
-                const int slot = nx % STAGES;
+                const int slot = nx % ST;
                 load_opk(sX + slot * OPK_BYTES, X, K, Rn, row0, (kt0 + nx) * BK, K, tid);
                 load_opk(sY + slot * OPK_BYTES, Y, K, cend, col0, (kt0 + nx) * BK, K, tid);
             }
             cp_async_commit();
         }
-        const char *bx = sX + (kt % STAGES) * OPK_BYTES, *by = sY + (kt % STAGES) * OPK_BYTES;
+        const char *bx = sX + (kt % ST) * OPK_BYTES, *by = sY + (kt % ST) * OPK_BYTES;
 #pragma unroll
         for (int kk = 0; kk < BK / 4; kk++) {
             double2 a[4], bq[NTL];
@@ -183,7 +189,8 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
 }
 
 // Out[i] = scale * dscale[c] * sum_s part[s][i]   (fixed order)
-// tri: only tiles with row tile >= col tile were computed; the rest is the conjugate transpose (Hermitian result)
+// tri = column tile width (0: off): only tiles reaching or below the diagonal were computed; the rest is the conjugate
+// transpose (Hermitian result)
 __global__ void k_splitk_reduce(const double2 *__restrict__ part, const int nsplit, const int64_t total, const int Cn,
                                 const double scale, const double *__restrict__ dscale, double2 *__restrict__ Out,
                                 const int tri, const int accumulate) {
@@ -192,7 +199,7 @@ __global__ void k_splitk_reduce(const double2 *__restrict__ part, const int nspl
         bool cj = false;
         if (tri) {
             const int r = (int)(i / Cn), c = (int)(i % Cn);
-            if (c / BN > r / BM) { src = (int64_t)c * Cn + r; cj = true; }
+            if ((c / tri) * tri > (r / BM) * BM + BM - 1) { src = (int64_t)c * Cn + r; cj = true; }   // tile not computed: mirror
         }
         double sr = 0.0, si = 0.0;
         for (int s = 0; s < nsplit; s++) {
@@ -273,7 +280,7 @@ __global__ void k_splitk_reduce_block_any(const double2 *__restrict__ part, cons
 // ---------------------------------------------------------------------------------------------- expand GEMM
 // BN_ x (WM x WN warps): 64 x (2 x 2) is the default tile; 56 x (4 x 1) exists because for some n extents it fills the
 // 148 x 3 CTA slots in whole waves where 64 leaves a half-empty tail wave (config 2: 1.68 -> 1.93 waves).
-template <int BN_, int WM, int WN, bool M3 = false>
+template <int BN_, int WM, int WN, bool M3 = false, int ST = STAGES>
 __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const double2 *__restrict__ A, const int Rn,
                                                           const double2 *__restrict__ Pm, const int K, const int64_t Nn,
                                                           double2 *Out, const double2 *Add,
@@ -282,7 +289,7 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
     constexpr int MTL = BM / (8 * WM), NTL = BN_ / (8 * WN);   // 8 x 8 DMMA tiles per warp along rows / columns
     constexpr int PROW = BN_ * 16 + 32, OPN = BK * PROW;
     static_assert(WM * WN * 32 == NTHREADS && MTL * 8 * WM == BM && NTL * 8 * WN == BN_, "warp layout");
-    char *sA = smem, *sP = smem + STAGES * OPK_BYTES;
+    char *sA = smem, *sP = smem + ST * OPK_BYTES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wr = (warp / WN) * (8 * MTL), wc = (warp % WN) * (8 * NTL);
     const int row0 = blockIdx.y * BM;
@@ -309,7 +316,7 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
             cp_async16(dst + kk * PROW + nn * 16, src, ok);
         }
     };
-    for (int s = 0; s < STAGES - 1; s++) {
+    for (int s = 0; s < ST - 1; s++) {
         if (s < nkt) {
             load_opk(sA + s * OPK_BYTES, A, K, Rn, row0, (int64_t)s * BK, K, tid);
             load_p(sP + s * OPN, s * BK);
@@ -319,18 +326,18 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
     const int fa = (lane >> 2) * 64 + (lane & 3) * 16;
     const int fp = (lane & 3) * PROW + (lane >> 2) * 16;
     for (int kt = 0; kt < nkt; kt++) {
-        cp_async_wait<STAGES - 2>();
+        cp_async_wait<ST - 2>();
         __syncthreads();
         {
-            const int nx = kt + STAGES - 1;
+            const int nx = kt + ST - 1;
             if (nx < nkt) {
-                const int slot = nx % STAGES;
+                const int slot = nx % ST;
                 load_opk(sA + slot * OPK_BYTES, A, K, Rn, row0, (int64_t)nx * BK, K, tid);
                 load_p(sP + slot * OPN, nx * BK);
             }
             cp_async_commit();
         }
-        const char *ba = sA + (kt % STAGES) * OPK_BYTES, *bp = sP + (kt % STAGES) * OPN;
+        const char *ba = sA + (kt % ST) * OPK_BYTES, *bp = sP + (kt % ST) * OPN;
 #pragma unroll
         for (int kk = 0; kk < BK / 4; kk++) {
             double2 a[MTL], bq[NTL];
@@ -428,10 +435,17 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     int bn = (!tri && Cn > 64 && pad48 * 100 < pad64 * 93) ? 48 : 64;  // measured: pays at 10 % padding (np = 288), not at 3.6 % (np = 864)
     // 3M scheme (three DMMAs per complex tile product; 64 x 48 tiles, its three accumulator sets leave no room for
     // 64 x 64): taken when 0.8 x its padded width beats the 4M choice and K is long enough to matter
-    const bool m3 = !tri && b->opt_gemm3m && K >= 512 && pad48 * 80 < (bn == 48 ? pad48 : pad64) * 100;
+    const bool m3 = b->opt_gemm3m && K >= 512 && (tri ? Cn >= 128 : pad48 * 80 < (bn == 48 ? pad48 : pad64) * 100);
     if (m3) bn = 48;
     const int tcol = (Cn + bn - 1) / bn;
-    const int tiles = tri ? trow * (trow + 1) / 2 : trow * tcol;
+    int tiles = trow * tcol;
+    if (tri) {
+        tiles = 0;
+        for (int tr = 0; tr < trow; tr++) {
+            const int nt = ((tr + 1) * BM - 1) / bn + 1;
+            tiles += nt < tcol ? nt : tcol;
+        }
+    }
     const size_t one = (size_t)Rn * Cn * 16;
     // Split K so that the grid fills whole waves of the SMs x 2 resident CTAs (184 registers x 128 threads):
     // among 1..6 waves take the smallest count whose fill tiles*nsplit / (waves*slots) is within 2 % of the best (stop at 97 %).
@@ -456,7 +470,8 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     if (per < 1) per = 1;
     nsplit = (ktiles + per - 1) / per;
     if (nsplit < 1) nsplit = 1;
-    const size_t smem = 2 * STAGES * OPK_BYTES;
+    constexpr int ST3 = 6;   // pipeline depth of the 3M kernels (2 CTAs per SM leave room for it)
+    const size_t smem = 2 * (m3 ? ST3 : STAGES) * OPK_BYTES;
     dim3 grid(tri ? tiles : tcol, tri ? 1 : trow, (unsigned)nsplit);
     jdft_prof_begin(b, JDFT_K_GEMM_DOTK, st);
 #define JDFT_DOTK_LAUNCH(...)                                                                                  \
@@ -465,9 +480,10 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
         k_gemm_dotk<__VA_ARGS__><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, \
                                                                (int)per, (double2 *)scratch);                  \
     } while (0)
-    if (tri) JDFT_DOTK_LAUNCH(true, true, 64);
-    else if (m3 && conjY) JDFT_DOTK_LAUNCH(true, false, 48, true);
-    else if (m3) JDFT_DOTK_LAUNCH(false, false, 48, true);
+    if (tri && m3) JDFT_DOTK_LAUNCH(true, true, 48, true, ST3);
+    else if (tri) JDFT_DOTK_LAUNCH(true, true, 64);
+    else if (m3 && conjY) JDFT_DOTK_LAUNCH(true, false, 48, true, ST3);
+    else if (m3) JDFT_DOTK_LAUNCH(false, false, 48, true, ST3);
     else if (conjY && bn == 48) JDFT_DOTK_LAUNCH(true, false, 48);
     else if (conjY) JDFT_DOTK_LAUNCH(true, false, 64);
     else if (bn == 48) JDFT_DOTK_LAUNCH(false, false, 48);
@@ -492,7 +508,7 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
         else
             k_splitk_reduce_block_any<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, Rn, Cn, nblk, scale, (const double2 *)dblock, (double2 *)Out);
     } else {
-        k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, total, Cn, scale, dscale, (double2 *)Out, tri, accumulate);
+        k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)scratch, (int)nsplit, total, Cn, scale, dscale, (double2 *)Out, tri ? bn : 0, accumulate);
     }
     jdft_prof_end(b, JDFT_K_REDUCE, st);
     JDFT_LAUNCH_CHECK("k_splitk_reduce");
@@ -511,12 +527,12 @@ int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double 
     };
     const bool narrow = fill(56) > fill(64) + 0.05;
     jdft_prof_begin(b, JDFT_K_GEMM_EXPAND, st);
-    if (b->opt_gemm3m && K >= 64) {   // 3M scheme: 64 x 48 tiles, 2 CTAs per SM (see k_gemm_dotk)
-        constexpr int BNX = 48;
-        const size_t smem = STAGES * (OPK_BYTES + BK * (BNX * 16 + 32));
-        JDFT_CUDA(ensure_smem(k_gemm_expand<BNX, 2, 2, true>, smem, b->device));
+    if (b->opt_gemm3m && K >= 320) {   // 3M scheme: 64 x 48 tiles, 2 CTAs per SM (see k_gemm_dotk); measured neutral at K = 288, -8 % at 384, -12 % at 864
+        constexpr int BNX = 48, ST3 = 6;
+        const size_t smem = ST3 * (OPK_BYTES + BK * (BNX * 16 + 32));
+        JDFT_CUDA(ensure_smem(k_gemm_expand<BNX, 2, 2, true, ST3>, smem, b->device));
         dim3 grid((unsigned)((Nn + BNX - 1) / BNX), (unsigned)rt);
-        k_gemm_expand<BNX, 2, 2, true><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, (const double2 *)Add, addscale);
+        k_gemm_expand<BNX, 2, 2, true, ST3><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, (const double2 *)Add, addscale);
     } else if (narrow) {
         constexpr int BNX = 56;
         const size_t smem = STAGES * (OPK_BYTES + BK * (BNX * 16 + 32));

@@ -27,6 +27,7 @@ struct jdft_basis {
     std::vector<double> ke;
     // pruning structure: planes p <-> m0 = m0lo + p; columns c of plane p <-> m1 = pl_m1lo[p] + (c - pl_cbase[p])
     int npl, m0lo, ncol, maxcol_per_plane;
+    int mmin[3], mmax[3];                     // extent of the sphere along each axis (signed m_d)
     std::vector<int> pl_m1lo, pl_cbase;       // [npl], [npl+1]
     std::vector<int> col_n0, col_m2lo;        // [ncol+1], [ncol]
     // device copies

@@ -1071,9 +1071,15 @@ int launch_cols_inv(const jdft_basis *b, const double2 *C, int nbt, double2 *W1,
     SPEC_SWITCH(L, b->opt_force_generic, {
         if constexpr (jcols::Cfg<LT>::ok) {
             using F = jcols::Cfg<LT>;
-            JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT>, F::smem, b->device));
             dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
-            jcols::k_cols_inv_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+            // pruned radix-8 first pass when no sphere point has |m2| >= 2 NB0 (rows [2 NB0, 6 NB0) empty)
+            if (F::R0 == 8 && b->opt_prune && b->mmin[2] > -2 * F::NB0 && b->mmax[2] < 2 * F::NB0) {
+                JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT, F::R0 == 8>, F::smem, b->device));
+                jcols::k_cols_inv_tuned<LT, F::R0 == 8><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+            } else {
+                JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT>, F::smem, b->device));
+                jcols::k_cols_inv_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+            }
         } else {
             JDFT_CUDA(ensure_smem(k_cols_inv<LT>, smem, b->device));
             k_cols_inv<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);

@@ -38,7 +38,13 @@
  * launch-time CUDA errors are returned, execution-time errors surface at the caller's next sync.
  *
  * The jdft_*_host entry points are the same operations taking HOST arrays: they allocate device
- * buffers, copy in, run the same kernels, copy out and synchronise (used for the end-to-end number).
+ * buffers, copy in, run the same kernels, copy out and synchronise (used for the end-to-end number);
+ * jdft_apply_H_host pipelines band chunks over three streams (H2D of chunk i+1, kernels of chunk i, D2H of
+ * chunk i-1 at once; pinned host arrays make the copies asynchronous).
+ *
+ * Concurrency.  A basis owns its workspace binding, its side streams and its events, so ONE stream (or host
+ * thread) at a time may run calls on a given basis.  Callers that want concurrent streams create one basis per
+ * stream (creation is cheap: an O(sphere) enumeration and a few small uploads).
  */
 #ifndef JDFT_H
 #define JDFT_H
@@ -158,6 +164,12 @@ int jdft_apply_H_host(jdft_basis *b, const double *Vloc_host, const double *P_ho
                       const double *D_host, int D_mode, const double *C_host, int nb, double *HC_host);
 int jdft_overlap_host(jdft_basis *b, const double *C1_host, int nb1, const double *C2_host, int nb2,
                       double *M_host);
+/* Resident operators: V_loc, P, D stay the same over the many H applications of an SCF iteration, so
+ * they are uploaded once into library-owned device buffers; jdft_apply_H_host_resident then moves only the bands in
+ * and H C out (chunk-pipelined on three streams like jdft_apply_H_host).  A later jdft_apply_H_host call replaces them. */
+int jdft_host_set_operators(jdft_basis *b, const double *Vloc_host, const double *P_host, int nproj,
+                            const double *D_host, int D_mode);
+int jdft_apply_H_host_resident(jdft_basis *b, const double *C_host, int nb, double *HC_host);
 
 /* ---- diagnostics ---------------------------------------------------------------------------------- */
 const char *jdft_last_error(void);

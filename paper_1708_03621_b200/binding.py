@@ -19,7 +19,7 @@ EXPORTS = [
     "jdft_basis_create", "jdft_basis_destroy", "jdft_basis_info", "jdft_basis_structure", "jdft_basis_export",
     "jdft_basis_device_maps", "jdft_workspace_bytes", "jdft_set_workspace", "jdft_set_option",
     "jdft_apply_I", "jdft_apply_Idag", "jdft_apply_J", "jdft_apply_L", "jdft_apply_O", "jdft_apply_Vnl",
-    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_apply_H_host", "jdft_overlap_host",
+    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_apply_H_host", "jdft_overlap_host", "jdft_host_set_operators", "jdft_apply_H_host_resident",
     "jdft_last_error", "jdft_launch_count", "jdft_profile_read", "jdft_version",
 ]
 
@@ -61,6 +61,8 @@ def _load():
     L.jdft_pcm_hessian.argtypes = [vp, vp, vp, ci, vp, vp]
     L.jdft_apply_H_host.argtypes = [vp, vp, vp, ci, vp, ci, vp, ci, vp]
     L.jdft_overlap_host.argtypes = [vp, vp, ci, vp, ci, vp]
+    L.jdft_host_set_operators.argtypes = [vp, vp, vp, ci, vp, ci]
+    L.jdft_apply_H_host_resident.argtypes = [vp, vp, ci, vp]
     L.jdft_last_error.restype = ctypes.c_char_p
     L.jdft_launch_count.argtypes = [ci]
     L.jdft_launch_count.restype = i64
@@ -374,6 +376,24 @@ def jdft_apply_H_host(basis, Vloc, P, D, C, HC):
         Dp = _host(D, torch.float64 if mode == 0 else torch.complex128, "D")
     _chk(_lib.jdft_apply_H_host(basis._h, _host(Vloc, torch.float64, "Vloc"), Pp, nproj, Dp, mode,
                                 _host(C, torch.complex128, "C"), nb, _host(HC, torch.complex128, "HC")))
+    return HC
+
+
+def jdft_host_set_operators(basis, Vloc, P, D):
+    """Upload V_loc, P, D once (HOST tensors); jdft_apply_H_host_resident then copies only the bands in and H C out."""
+    if P is None or P.shape[0] == 0:
+        Pp, nproj, Dp, mode = None, 0, None, 0
+    else:
+        nproj = int(P.shape[0])
+        mode = 0 if D.dim() == 1 else (1 if D.dim() == 2 else int(D.shape[1]))
+        Pp = _host(P, torch.complex128, "P")
+        Dp = _host(D, torch.float64 if mode == 0 else torch.complex128, "D")
+    _chk(_lib.jdft_host_set_operators(basis._h, _host(Vloc, torch.float64, "Vloc"), Pp, nproj, Dp, mode))
+
+
+def jdft_apply_H_host_resident(basis, C, HC):
+    _chk(_lib.jdft_apply_H_host_resident(basis._h, _host(C, torch.complex128, "C"), int(C.shape[0]),
+                                         _host(HC, torch.complex128, "HC")))
     return HC
 
 

@@ -206,6 +206,105 @@ int host_buf(jdft_basis *b, int slot, size_t bytes, void **out) {
 }
 }  // namespace
 
+namespace {
+
+// streams / events of the HOST-buffer pipeline, created on first use (all non-blocking: no legacy-stream coupling)
+int host_streams(jdft_basis *b, int nchunk) {
+    for (int i = 0; i < 3; i++)
+        if (!b->hs[i]) JDFT_CUDA(cudaStreamCreateWithFlags(&b->hs[i], cudaStreamNonBlocking));
+    while ((int)b->hev.size() < 2 * nchunk + 2) {
+        cudaEvent_t e;
+        JDFT_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        b->hev.push_back(e);
+    }
+    return JDFT_OK;
+}
+
+// H C for HOST bands through device copies, pipelined over band chunks: the H2D copy of chunk i+1, the kernels of chunk i
+// and the D2H copy of chunk i-1 run at the same time on three streams (PCIe is full duplex).  dV / dP / dD are DEVICE
+// operands; with upload_ops they are first filled from the HOST arrays Vh / Ph / Dh, ordered so that the FFT pipeline of
+// chunk 0 starts as soon as V_loc and the chunk have landed while the (larger) projector block is still in flight.
+int host_H_pipeline(jdft_basis *b, bool upload_ops, const double *Vh, const double *Ph, const double *Dh, double *dV,
+                    double *dP, double *dD, int nproj, int D_mode, size_t vb, size_t pb, size_t db, const double *C,
+                    int nb, double *HC, const char *who) {
+    const int64_t nG = b->nG;
+    const size_t cb = (size_t)nb * nG * 16;
+    void *dCv, *dHCv, *dW;
+    int rc;
+    if ((rc = host_buf(b, 0, cb, &dCv)) || (rc = host_buf(b, 1, cb, &dHCv))) return rc;
+    double *dC = (double *)dCv, *dHC = (double *)dHCv;
+    int nchunk = (nb + 127) / 128;                       // chunks of <= 128 bands, at most 8 of them
+    if (nchunk > 8) nchunk = 8;
+    const int nbc = (nb + nchunk - 1) / nchunk;
+    nchunk = (nb + nbc - 1) / nbc;
+    if ((rc = host_streams(b, nchunk))) return rc;
+    void *saved_ws = b->ws;
+    size_t saved_bytes = b->ws_bytes;
+    if (!b->ws) {
+        size_t need = jdft_workspace_bytes(b, nbc < 64 ? nbc : 64, nproj > nbc ? nproj : nbc);
+        if ((rc = host_buf(b, 5, need, &dW))) return rc;
+        b->ws = dW;
+        b->ws_bytes = need;
+    }
+    // workspace split as in the fork/join path of jdft_apply_H: GEMM scratch in front, FFT intermediates behind
+    const size_t bsz = align_up((size_t)nbc * nproj * 16);
+    size_t part_bytes = b->ws_bytes / 4 < ((size_t)64 << 20) ? b->ws_bytes / 4 : ((size_t)64 << 20);
+    part_bytes &= ~(size_t)255;
+    const size_t gemm_bytes = nproj > 0 ? 2 * bsz + part_bytes : 0;
+    if ((nproj > 0 && part_bytes < (size_t)nbc * nproj * 16) || jdft_band_batch(b, nbc, gemm_bytes) == 0) {
+        b->ws = saved_ws;
+        b->ws_bytes = saved_bytes;
+        return jdft_fail(JDFT_EWORKSPACE, "%s: workspace too small", who);
+    }
+    char *ws = (char *)b->ws;
+    double *B1 = (double *)ws, *B2 = (double *)(ws + bsz);
+    cudaStream_t sin = b->hs[0], sc = b->hs[1], sout = b->hs[2];
+    cudaEvent_t evV = b->hev[0], evOps = b->hev[1];
+    cudaError_t e = cudaSuccess;
+    rc = JDFT_OK;
+    for (int i = 0; i < nchunk && e == cudaSuccess && !rc; i++) {
+        const int b0 = i * nbc, nbt = nb - b0 < nbc ? nb - b0 : nbc;
+        const size_t off = (size_t)b0 * nG * 2;          // in doubles
+        cudaEvent_t evIn = b->hev[2 + 2 * i], evDone = b->hev[3 + 2 * i];
+        if (i == 0 && upload_ops) {
+            e = cudaMemcpyAsync(dV, Vh, vb, cudaMemcpyHostToDevice, sin);
+            if (e == cudaSuccess) e = cudaEventRecord(evV, sin);
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(dC + off, C + off, (size_t)nbt * nG * 16, cudaMemcpyHostToDevice, sin);
+        if (e == cudaSuccess) e = cudaEventRecord(evIn, sin);
+        if (i == 0 && upload_ops && nproj > 0) {
+            if (e == cudaSuccess) e = cudaMemcpyAsync(dP, Ph, pb, cudaMemcpyHostToDevice, sin);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(dD, Dh, db, cudaMemcpyHostToDevice, sin);
+            if (e == cudaSuccess) e = cudaEventRecord(evOps, sin);
+        }
+        if (e == cudaSuccess && i == 0 && upload_ops) e = cudaStreamWaitEvent(sc, evV, 0);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(sc, evIn, 0);
+        if (e != cudaSuccess) break;
+        rc = jdft_local_H(b, dV, dC + off, nbt, dHC + off, sc, gemm_bytes);
+        if (!rc && nproj > 0) {
+            if (i == 0 && upload_ops) e = cudaStreamWaitEvent(sc, evOps, 0);
+            const double *Bd = B1;
+            if (e == cudaSuccess) rc = project_D(b, dP, nproj, dD, D_mode, dC + off, nbt, 1.0, B1, B2, ws + 2 * bsz, part_bytes, sc, &Bd);
+            if (e == cudaSuccess && !rc) rc = jdft_gemm_expand(b, Bd, nbt, dP, nproj, nG, dHC + off, 1, sc);
+        }
+        if (e == cudaSuccess && !rc) e = cudaEventRecord(evDone, sc);
+        if (e == cudaSuccess && !rc) e = cudaStreamWaitEvent(sout, evDone, 0);
+        if (e == cudaSuccess && !rc) e = cudaMemcpyAsync(HC + off, dHC + off, (size_t)nbt * nG * 16, cudaMemcpyDeviceToHost, sout);
+    }
+    b->ws = saved_ws;
+    b->ws_bytes = saved_bytes;
+    // always drain the three streams before returning (also on error: the caller may free its buffers)
+    cudaError_t e1 = cudaStreamSynchronize(sin), e2 = cudaStreamSynchronize(sc), e3 = cudaStreamSynchronize(sout);
+    if (rc) return rc;
+    if (e != cudaSuccess) return jdft_cuda_fail(e, who);
+    if (e1 != cudaSuccess) return jdft_cuda_fail(e1, who);
+    if (e2 != cudaSuccess) return jdft_cuda_fail(e2, who);
+    if (e3 != cudaSuccess) return jdft_cuda_fail(e3, who);
+    return JDFT_OK;
+}
+
+}  // namespace
+
 extern "C" int jdft_apply_H_host(jdft_basis *b, const double *Vloc, const double *P, int nproj, const double *D,
                                  int D_mode, const double *C, int nb, double *HC) {
     if (!b) return jdft_fail(JDFT_EINVAL, "apply_H_host: null basis");
@@ -213,67 +312,51 @@ extern "C" int jdft_apply_H_host(jdft_basis *b, const double *Vloc, const double
     if (!Vloc || (nb > 0 && (!C || !HC)) || (nproj > 0 && (!P || !D))) return jdft_fail(JDFT_EINVAL, "apply_H_host: null pointer");
     if (nb == 0) return JDFT_OK;
     JDFT_CUDA(cudaSetDevice(b->device));
-    const size_t cb = (size_t)nb * b->nG * 16, vb = (size_t)b->N * 8, pb = (size_t)nproj * b->nG * 16;
+    const size_t vb = (size_t)b->N * 8, pb = (size_t)nproj * b->nG * 16;
     const size_t db = D_mode == 0 ? (size_t)nproj * 8 : (D_mode == 1 ? (size_t)nproj * nproj * 16 : (size_t)nproj * D_mode * 16);
-    void *dC, *dHC, *dV, *dP, *dD, *dW;
+    void *dV, *dP, *dD;
     int rc;
-    if ((rc = host_buf(b, 0, cb, &dC)) || (rc = host_buf(b, 1, cb, &dHC)) || (rc = host_buf(b, 2, vb, &dV)) ||
-        (rc = host_buf(b, 3, pb, &dP)) || (rc = host_buf(b, 4, db, &dD)))
-        return rc;
-    void *saved_ws = b->ws;
-    size_t saved_bytes = b->ws_bytes;
-    if (!b->ws) {
-        const int rows = nproj > nb ? nproj : nb;
-        size_t need = jdft_workspace_bytes(b, 8, rows);
-        if ((rc = host_buf(b, 5, need, &dW))) return rc;
-        b->ws = dW;
-        b->ws_bytes = need;
+    if ((rc = host_buf(b, 2, vb, &dV)) || (rc = host_buf(b, 3, pb, &dP)) || (rc = host_buf(b, 4, db, &dD))) return rc;
+    b->h_ops_set = 0;   // the resident operators (if any) have just been overwritten
+    return host_H_pipeline(b, true, Vloc, P, D, (double *)dV, (double *)dP, (double *)dD, nproj, D_mode, vb, pb, db, C, nb, HC,
+                           "apply_H_host");
+}
+
+// Resident operators: V_loc, P and D are uploaded ONCE (they stay the same over the many H applications of one SCF
+// iteration); jdft_apply_H_host_resident then moves only the bands in and H C out.
+extern "C" int jdft_host_set_operators(jdft_basis *b, const double *Vloc, const double *P, int nproj, const double *D,
+                                       int D_mode) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "host_set_operators: null basis");
+    if (nproj < 0 || D_mode < 0 || (D_mode >= 2 && nproj % D_mode != 0)) return jdft_fail(JDFT_EINVAL, "host_set_operators: bad size or mode");
+    if (!Vloc || (nproj > 0 && (!P || !D))) return jdft_fail(JDFT_EINVAL, "host_set_operators: null pointer");
+    JDFT_CUDA(cudaSetDevice(b->device));
+    const size_t vb = (size_t)b->N * 8, pb = (size_t)nproj * b->nG * 16;
+    const size_t db = D_mode == 0 ? (size_t)nproj * 8 : (D_mode == 1 ? (size_t)nproj * nproj * 16 : (size_t)nproj * D_mode * 16);
+    void *dV, *dP, *dD;
+    int rc;
+    if ((rc = host_buf(b, 2, vb, &dV)) || (rc = host_buf(b, 3, pb, &dP)) || (rc = host_buf(b, 4, db, &dD))) return rc;
+    if ((rc = host_streams(b, 1))) return rc;
+    b->h_ops_set = 0;
+    JDFT_CUDA(cudaMemcpyAsync(dV, Vloc, vb, cudaMemcpyHostToDevice, b->hs[0]));
+    if (nproj > 0) {
+        JDFT_CUDA(cudaMemcpyAsync(dP, P, pb, cudaMemcpyHostToDevice, b->hs[0]));
+        JDFT_CUDA(cudaMemcpyAsync(dD, D, db, cudaMemcpyHostToDevice, b->hs[0]));
     }
-    // Copy-in on the basis' side stream in the order the kernels need the data (C, Vloc, then P, D); the FFT pipeline
-    // starts as soon as C and Vloc have landed and runs while the (larger) projector block is still in flight; the
-    // projector GEMMs wait for the second event.  Pinned host buffers make the copies truly asynchronous.
-    cudaStream_t st = 0, cp = b->side ? b->side : (cudaStream_t)0;
-    cudaError_t e = cudaMemcpyAsync(dC, C, cb, cudaMemcpyHostToDevice, cp);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dV, Vloc, vb, cudaMemcpyHostToDevice, cp);
-    if (e == cudaSuccess && cp != st) e = cudaEventRecord(b->ev_fork, cp);
-    if (e == cudaSuccess && nproj > 0) e = cudaMemcpyAsync(dP, P, pb, cudaMemcpyHostToDevice, cp);
-    if (e == cudaSuccess && nproj > 0) e = cudaMemcpyAsync(dD, D, db, cudaMemcpyHostToDevice, cp);
-    if (e == cudaSuccess && cp != st) e = cudaEventRecord(b->ev_join, cp);
-    if (e == cudaSuccess && cp != st) e = cudaStreamWaitEvent(st, b->ev_fork, 0);
-    rc = e == cudaSuccess ? JDFT_OK : jdft_cuda_fail(e, "apply_H_host H2D");
-    if (!rc) {
-        if (nproj == 0) {
-            rc = jdft_local_H(b, (const double *)dV, (const double *)dC, nb, (double *)dHC, st);
-        } else {
-            // same split of the workspace as the fork/join path of jdft_apply_H: GEMM scratch in front, FFT behind
-            const size_t bsz = align_up((size_t)nb * nproj * 16);
-            size_t part_bytes = b->ws_bytes / 4 < ((size_t)64 << 20) ? b->ws_bytes / 4 : ((size_t)64 << 20);
-            part_bytes &= ~(size_t)255;
-            const size_t gemm_bytes = 2 * bsz + part_bytes;
-            if (part_bytes < (size_t)nb * nproj * 16 || jdft_band_batch(b, nb, gemm_bytes) == 0) {
-                rc = jdft_fail(JDFT_EWORKSPACE, "apply_H_host: workspace too small");
-            } else {
-                char *ws = (char *)b->ws;
-                double *B1 = (double *)ws, *B2 = (double *)(ws + bsz);
-                rc = jdft_local_H(b, (const double *)dV, (const double *)dC, nb, (double *)dHC, st, gemm_bytes);
-                if (cp != st) {
-                    cudaError_t e2 = cudaStreamWaitEvent(st, b->ev_join, 0);
-                    if (!rc && e2 != cudaSuccess) rc = jdft_cuda_fail(e2, "apply_H_host join");
-                }
-                const double *Bd = B1;
-                if (!rc) rc = project_D(b, (const double *)dP, nproj, (const double *)dD, D_mode, (const double *)dC, nb, 1.0, B1, B2,
-                                        ws + 2 * bsz, part_bytes, st, &Bd);
-                if (!rc) rc = jdft_gemm_expand(b, Bd, nb, (const double *)dP, nproj, b->nG, (double *)dHC, 1, st);
-            }
-        }
-    }
-    b->ws = saved_ws;
-    b->ws_bytes = saved_bytes;
-    if (rc) { cudaStreamSynchronize(cp); cudaStreamSynchronize(st); return rc; }
-    JDFT_CUDA(cudaMemcpyAsync(HC, dHC, cb, cudaMemcpyDeviceToHost, st));
-    JDFT_CUDA(cudaStreamSynchronize(st));
-    JDFT_CUDA(cudaStreamSynchronize(cp));
+    JDFT_CUDA(cudaStreamSynchronize(b->hs[0]));
+    b->h_ops_set = 1;
+    b->h_nproj = nproj;
+    b->h_D_mode = D_mode;
     return JDFT_OK;
+}
+
+extern "C" int jdft_apply_H_host_resident(jdft_basis *b, const double *C, int nb, double *HC) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "apply_H_host_resident: null basis");
+    if (!b->h_ops_set) return jdft_fail(JDFT_EINVAL, "apply_H_host_resident: call jdft_host_set_operators first");
+    if (nb < 0 || (nb > 0 && (!C || !HC))) return jdft_fail(JDFT_EINVAL, "apply_H_host_resident: bad size or null pointer");
+    if (nb == 0) return JDFT_OK;
+    JDFT_CUDA(cudaSetDevice(b->device));
+    return host_H_pipeline(b, false, nullptr, nullptr, nullptr, (double *)b->hb[2], (double *)b->hb[3], (double *)b->hb[4],
+                           b->h_nproj, b->h_D_mode, 0, 0, 0, C, nb, HC, "apply_H_host_resident");
 }
 
 extern "C" int jdft_overlap_host(jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M) {
@@ -282,10 +365,14 @@ extern "C" int jdft_overlap_host(jdft_basis *b, const double *C1, int nb1, const
     if (nb1 == 0 || nb2 == 0) return JDFT_OK;
     if (!C1 || !C2 || !M) return jdft_fail(JDFT_EINVAL, "overlap_host: null pointer");
     JDFT_CUDA(cudaSetDevice(b->device));
+    const bool same = C1 == C2 && nb1 == nb2;   // one upload; the device call then takes the Hermitian-triangle path
     const size_t b1 = (size_t)nb1 * b->nG * 16, b2 = (size_t)nb2 * b->nG * 16, mb = (size_t)nb1 * nb2 * 16;
     void *d1, *d2, *dM, *dW;
     int rc;
-    if ((rc = host_buf(b, 0, b1, &d1)) || (rc = host_buf(b, 1, b2, &d2)) || (rc = host_buf(b, 6, mb, &dM))) return rc;
+    if ((rc = host_buf(b, 0, b1, &d1)) || (rc = host_buf(b, 6, mb, &dM))) return rc;
+    d2 = d1;
+    if (!same && (rc = host_buf(b, 1, b2, &d2))) return rc;
+    if ((rc = host_streams(b, 1))) return rc;
     void *saved_ws = b->ws;
     size_t saved_bytes = b->ws_bytes;
     if (!b->ws) {
@@ -294,14 +381,14 @@ extern "C" int jdft_overlap_host(jdft_basis *b, const double *C1, int nb1, const
         b->ws = dW;
         b->ws_bytes = need;
     }
-    cudaStream_t st = 0;
+    cudaStream_t st = b->hs[1];
     cudaError_t e = cudaMemcpyAsync(d1, C1, b1, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d2, C2, b2, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && !same) e = cudaMemcpyAsync(d2, C2, b2, cudaMemcpyHostToDevice, st);
     rc = e == cudaSuccess ? jdft_overlap(b, (const double *)d1, nb1, (const double *)d2, nb2, (double *)dM, st)
                           : jdft_cuda_fail(e, "overlap_host H2D");
     b->ws = saved_ws;
     b->ws_bytes = saved_bytes;
-    if (rc) return rc;
+    if (rc) { cudaStreamSynchronize(st); return rc; }
     JDFT_CUDA(cudaMemcpyAsync(M, dM, mb, cudaMemcpyDeviceToHost, st));
     JDFT_CUDA(cudaStreamSynchronize(st));
     return JDFT_OK;

@@ -107,6 +107,8 @@ extern "C" int jdft_basis_destroy(jdft_basis *b) {
     if (b->ev_fork) cudaEventDestroy(b->ev_fork);
     if (b->ev_join) cudaEventDestroy(b->ev_join);
     for (int i = 0; i < 8; i++) cudaFree(b->hb[i]);
+    for (int i = 0; i < 3; i++) if (b->hs[i]) cudaStreamDestroy(b->hs[i]);
+    for (cudaEvent_t e : b->hev) cudaEventDestroy(e);
     for (cudaEvent_t e : b->prof_ev) cudaEventDestroy(e);
     delete b;
     return JDFT_OK;
@@ -136,6 +138,8 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     b->d_rowcol = nullptr; b->d_planeof = nullptr;
     for (int d = 0; d < 3; d++) b->d_tw[d] = nullptr;
     for (int i = 0; i < 8; i++) { b->hb[i] = nullptr; b->hb_bytes[i] = 0; }
+    for (int i = 0; i < 3; i++) b->hs[i] = nullptr;
+    b->h_ops_set = 0; b->h_nproj = 0; b->h_D_mode = 0;
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
     b->opt_profile_kernel = 0; b->prof_used = 0;
     b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_gemm3m = 1; b->opt_tma = 0; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;

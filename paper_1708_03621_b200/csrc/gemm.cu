@@ -35,12 +35,13 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, const double a, con
 }
 
 // load one stage of a K-contiguous operand: rows [row0, row0+64) of M [nrows][ld], k in [k0, k0+BK), zero beyond kend/nrows
+template <int BKT = BK>
 __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld, int nrows, int row0, int64_t k0,
                                          int64_t kend, int tid) {
 #pragma unroll
-    for (int i = 0; i < (64 * BK) / NTHREADS; i++) {
+    for (int i = 0; i < (64 * BKT) / NTHREADS; i++) {
         const int e = tid + i * NTHREADS;
-        const int r = e / BK, kk = e % BK;
+        const int r = e / BKT, kk = e % BKT;
         const int64_t k = k0 + kk;
         const bool ok = (row0 + r < nrows) && (k < kend);
         const double2 *src = ok ? M + (size_t)(row0 + r) * ld + k : M;
@@ -55,12 +56,13 @@ __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld
 // (three accumulator sets; the two operand sums cost 1 + 2/MT DADD per fragment).  Normwise as accurate as the 4M
 // scheme (Higham, Accuracy and Stability, ch. 23: 3M is normwise stable), which is what the per-band relative L2
 // tolerance measures; 25 % fewer tensor instructions.
-template <bool CONJY, bool TRI, int BN_, bool M3 = false, int ST = STAGES>
+template <bool CONJY, bool TRI, int BN_, bool M3 = false, int ST = STAGES, int BKT = BK>
 __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
                                                         const double2 *__restrict__ Y, const int Cn, const int64_t K,
                                                         const int ktiles_per_split, double2 *__restrict__ part) {
     extern __shared__ __align__(16) char smem[];
-    char *sX = smem, *sY = smem + ST * OPK_BYTES;
+    constexpr int OPKT = (BKT / 4) * KBLK_BYTES;   // one stage of a K-contiguous operand
+    char *sX = smem, *sY = smem + ST * OPKT;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NTL = BN_ / 16;   // 8-wide DMMA tiles per warp along the columns
     const int wr = (warp >> 1) * 32, wc = (warp & 1) * (BN_ / 2);
@@ -82,7 +84,7 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
     const int row0 = tr * BM, col0 = tc * BN_;
     // rows of Y this tile owns (the loader fills the rest of its 64 rows with zeros); 64: exactly the original code path
     const int cend = BN_ == 64 ? Cn : min(Cn, col0 + BN_);
-    const int64_t ktiles = (K + BK - 1) / BK;
+    const int64_t ktiles = (K + BKT - 1) / BKT;
     const int64_t kt0 = (int64_t)blockIdx.z * ktiles_per_split;
     int64_t kt1 = kt0 + ktiles_per_split;
     if (kt1 > ktiles) kt1 = ktiles;
@@ -100,8 +102,8 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
 
     for (int s = 0; s < ST - 1; s++) {
         if (s < nkt) {
-            load_opk(sX + s * OPK_BYTES, X, K, Rn, row0, (kt0 + s) * BK, K, tid);
-            load_opk(sY + s * OPK_BYTES, Y, K, cend, col0, (kt0 + s) * BK, K, tid);
+            load_opk<BKT>(sX + s * OPKT, X, K, Rn, row0, (kt0 + s) * BKT, K, tid);
+            load_opk<BKT>(sY + s * OPKT, Y, K, cend, col0, (kt0 + s) * BKT, K, tid);
         }
         cp_async_commit();
     }
@@ -113,14 +115,14 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
             const int nx = kt + ST - 1;
             if (nx < nkt) {
                 const int slot = nx % ST;
-                load_opk(sX + slot * OPK_BYTES, X, K, Rn, row0, (kt0 + nx) * BK, K, tid);
-                load_opk(sY + slot * OPK_BYTES, Y, K, cend, col0, (kt0 + nx) * BK, K, tid);
+                load_opk<BKT>(sX + slot * OPKT, X, K, Rn, row0, (kt0 + nx) * BKT, K, tid);
+                load_opk<BKT>(sY + slot * OPKT, Y, K, cend, col0, (kt0 + nx) * BKT, K, tid);
             }
             cp_async_commit();
         }
-        const char *bx = sX + (kt % ST) * OPK_BYTES, *by = sY + (kt % ST) * OPK_BYTES;
+        const char *bx = sX + (kt % ST) * OPKT, *by = sY + (kt % ST) * OPKT;
 #pragma unroll
-        for (int kk = 0; kk < BK / 4; kk++) {
+        for (int kk = 0; kk < BKT / 4; kk++) {
             double2 a[4], bq[NTL];
 #pragma unroll
             for (int i = 0; i < 4; i++)
@@ -426,7 +428,6 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     if (Rn <= 0 || Cn <= 0) return JDFT_OK;
     if (dblock && (nblk < 1 || Cn % nblk != 0 || dscale || accumulate))
         return jdft_fail(JDFT_EINVAL, "gemm: block-diagonal D needs nproj %% block == 0");
-    const int64_t ktiles = (K + BK - 1) / BK;
     // X^+ X is Hermitian: compute the lower-triangle tiles only and mirror them in the reduction
     const int tri = (X == Y && Rn == Cn && conjY && !dscale && !dblock && BM == BN) ? 1 : 0;
     const int trow = (Rn + BM - 1) / BM;
@@ -437,6 +438,10 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     // 64 x 64): taken when 0.8 x its padded width beats the 4M choice and K is long enough to matter
     const bool m3 = b->opt_gemm3m && K >= 512 && (tri ? Cn >= 128 : pad48 * 80 < (bn == 48 ? pad48 : pad64) * 100);
     if (m3) bn = 48;
+    // the 3M kernels run k-tiles of 16 in a 3-stage pipeline (half the barriers per DMMA of the 8-deep 4-stage 4M kernels)
+    constexpr int ST3 = 3, BK3 = 16;
+    const int bk = m3 ? BK3 : BK;
+    const int64_t ktiles = (K + bk - 1) / bk;
     const int tcol = (Cn + bn - 1) / bn;
     int tiles = trow * tcol;
     if (tri) {
@@ -450,7 +455,8 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     // Split K so that the grid fills whole waves of the SMs x 2 resident CTAs (184 registers x 128 threads):
     // among 1..6 waves take the smallest count whose fill tiles*nsplit / (waves*slots) is within 2 % of the best (stop at 97 %).
     const int64_t slots = (int64_t)b->num_sms * 2;
-    const int64_t max_by_k = ktiles / 16 > 0 ? ktiles / 16 : 1;              // at least 16 k-tiles (128 k) per slice
+    const int64_t min_kt = 128 / bk;                                         // at least 128 k per slice
+    const int64_t max_by_k = ktiles / min_kt > 0 ? ktiles / min_kt : 1;
     const int64_t max_by_ws = (int64_t)(scratch_bytes / one);
     if (max_by_ws < 1) return jdft_fail(JDFT_EWORKSPACE, "gemm: workspace too small for a %d x %d result", Rn, Cn);
     int64_t nsplit = 1;
@@ -470,8 +476,7 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     if (per < 1) per = 1;
     nsplit = (ktiles + per - 1) / per;
     if (nsplit < 1) nsplit = 1;
-    constexpr int ST3 = 6;   // pipeline depth of the 3M kernels (2 CTAs per SM leave room for it)
-    const size_t smem = 2 * (m3 ? ST3 : STAGES) * OPK_BYTES;
+    const size_t smem = m3 ? 2 * ST3 * (BK3 / 4) * KBLK_BYTES : 2 * STAGES * OPK_BYTES;
     dim3 grid(tri ? tiles : tcol, tri ? 1 : trow, (unsigned)nsplit);
     jdft_prof_begin(b, JDFT_K_GEMM_DOTK, st);
 #define JDFT_DOTK_LAUNCH(...)                                                                                  \
@@ -480,10 +485,10 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
         k_gemm_dotk<__VA_ARGS__><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, \
                                                                (int)per, (double2 *)scratch);                  \
     } while (0)
-    if (tri && m3) JDFT_DOTK_LAUNCH(true, true, 48, true, ST3);
+    if (tri && m3) JDFT_DOTK_LAUNCH(true, true, 48, true, ST3, BK3);
     else if (tri) JDFT_DOTK_LAUNCH(true, true, 64);
-    else if (m3 && conjY) JDFT_DOTK_LAUNCH(true, false, 48, true, ST3);
-    else if (m3) JDFT_DOTK_LAUNCH(false, false, 48, true, ST3);
+    else if (m3 && conjY) JDFT_DOTK_LAUNCH(true, false, 48, true, ST3, BK3);
+    else if (m3) JDFT_DOTK_LAUNCH(false, false, 48, true, ST3, BK3);
     else if (conjY && bn == 48) JDFT_DOTK_LAUNCH(true, false, 48);
     else if (conjY) JDFT_DOTK_LAUNCH(true, false, 64);
     else if (bn == 48) JDFT_DOTK_LAUNCH(false, false, 48);

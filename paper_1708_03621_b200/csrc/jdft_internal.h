@@ -60,6 +60,9 @@ struct jdft_basis {
     // cached device buffers of the *_host entry points (library-owned, grow-only)
     void *hb[8];
     size_t hb_bytes[8];
+    cudaStream_t hs[3];                       // H2D, compute and D2H streams of the *_host pipeline (created on first use)
+    std::vector<cudaEvent_t> hev;
+    int h_ops_set, h_nproj, h_D_mode;         // resident operators of jdft_host_set_operators (in hb[2..4])
 };
 
 // kernel ids for the "profile_kernel" option

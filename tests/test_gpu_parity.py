@@ -213,6 +213,38 @@ def test_host_variants(case, jd):
     assert rel_err_per_band(got.T, case.rb.overlap(case.C, case.C).T) <= TOL
 
 
+def test_host_pipeline_chunks_and_resident_operators(ref, jd):
+    """jdft_apply_H_host pipelines band chunks over three streams; 300 bands of a small box span three chunks with a
+    ragged last one.  jdft_host_set_operators + jdft_apply_H_host_resident give the same result; a dense and a
+    block-diagonal D go through the same path; without a caller workspace the library allocates its own."""
+    c = Case(ref, jd, 101, nb=300)
+    want = c.rb.apply_H(c.V, c.P, c.D, c.C)
+    Vt, Pt, Ct = torch.from_numpy(c.V.reshape(-1).copy()), torch.from_numpy(c.P), torch.from_numpy(c.C)
+    for pinned in (False, True):
+        HC = torch.empty(c.C.shape, dtype=torch.complex128)
+        if pinned:
+            HC = HC.pin_memory()
+        jd.jdft_apply_H_host(c.gb, Vt, Pt, torch.from_numpy(c.D), Ct, HC)
+        assert rel_err_per_band(HC.numpy(), want) <= TOL
+    jd.jdft_host_set_operators(c.gb, Vt, Pt, torch.from_numpy(c.D))
+    HC2 = torch.empty(c.C.shape, dtype=torch.complex128).pin_memory()
+    jd.jdft_apply_H_host_resident(c.gb, Ct, HC2)
+    assert rel_err_per_band(HC2.numpy(), want) <= TOL
+    rng = np.random.default_rng(3)
+    n = c.P.shape[0]
+    A = rng.standard_normal((n // 4, 4, 4)) + 1j * rng.standard_normal((n // 4, 4, 4))
+    Db = np.ascontiguousarray(A + A.conj().transpose(0, 2, 1))
+    jd.jdft_set_workspace(c.gb, None)                       # library-owned workspace
+    jd.jdft_apply_H_host(c.gb, Vt, Pt, torch.from_numpy(Db), Ct, HC2)
+    assert rel_err_per_band(HC2.numpy(), c.rb.apply_H(c.V, c.P, Db, c.C)) <= TOL
+    with pytest.raises(jd.JdftError):                       # apply_H_host replaced the resident operators
+        jd.jdft_apply_H_host_resident(c.gb, Ct, HC2)
+    # no projectors
+    jd.jdft_host_set_operators(c.gb, Vt, None, None)
+    jd.jdft_apply_H_host_resident(c.gb, Ct, HC2)
+    assert rel_err_per_band(HC2.numpy(), c.rb.apply_H(c.V, None, None, c.C)) <= TOL
+
+
 # ------------------------------------------------------------------------------------------ GPU-side properties
 
 def test_generic_fft_path_matches(ref, jd):

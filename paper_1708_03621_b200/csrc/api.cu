@@ -88,13 +88,10 @@ extern "C" int jdft_project(const jdft_basis *b, const double *P, int nproj, con
     return jdft_gemm_dotk(b, C, nb, P, nproj, b->nG, 1, 1.0, nullptr, Bproj, b->ws, b->ws_bytes, (cudaStream_t)s);
 }
 
-extern "C" int jdft_apply_H(const jdft_basis *b, const double *Vloc, const double *P, int nproj, const double *D,
-                            int D_mode, const double *C, int nb, double *HC, jdft_stream s) {
-    int rc = check_vnl_args(b, P, nproj, D, D_mode, C, nb, HC, "apply_H");
-    if (rc) return rc;
-    if (!Vloc) return jdft_fail(JDFT_EINVAL, "apply_H: null Vloc");
-    if (nb == 0) return JDFT_OK;
-    cudaStream_t st = (cudaStream_t)s;
+namespace {
+int apply_H_launch(const jdft_basis *b, const double *Vloc, const double *P, int nproj, const double *D, int D_mode,
+                   const double *C, int nb, double *HC, cudaStream_t st) {
+    int rc;
     if (nproj == 0) return jdft_local_H(b, Vloc, C, nb, HC, st);
     // Fork/join: B = D P^+ C (DMMA pipe) runs on the basis' side stream while the FFT pipeline (shared-memory / FP64
     // pipes) runs on the caller's stream; HC += P B follows both.  Needs separate workspace regions for the two.
@@ -121,6 +118,72 @@ extern "C" int jdft_apply_H(const jdft_basis *b, const double *Vloc, const doubl
     if (rc_side) return rc_side;
     if (rc) return rc;
     return jdft_gemm_expand(b, Bd, nb, P, nproj, b->nG, HC, 1, st);
+}
+
+}  // namespace
+
+// CUDA-graph replay of small calls (option "graph"; automatic when nb * N <= 4 Mi points, where the ten launches of one
+// call cost more than their kernels): the second call with the same arguments and workspace captures the launch
+// sequence on a private stream; later calls replay it with one cudaGraphLaunch.  Capture failures fall back to direct
+// launches for good.  Off while per-kernel profiling is on (events inside a graph cannot be timed).
+extern "C" int jdft_apply_H(const jdft_basis *cb, const double *Vloc, const double *P, int nproj, const double *D,
+                            int D_mode, const double *C, int nb, double *HC, jdft_stream s) {
+    int rc = check_vnl_args(cb, P, nproj, D, D_mode, C, nb, HC, "apply_H");
+    if (rc) return rc;
+    if (!Vloc) return jdft_fail(JDFT_EINVAL, "apply_H: null Vloc");
+    if (nb == 0) return JDFT_OK;
+    cudaStream_t st = (cudaStream_t)s;
+    const bool want_graph = cb->opt_graph > 0 || (cb->opt_graph < 0 && (int64_t)nb * cb->N <= ((int64_t)4 << 20));
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (want_graph) cudaStreamIsCapturing(st, &cap);
+    if (!want_graph || cb->opt_profile_kernel || cb->opt_overlap || cap != cudaStreamCaptureStatusNone)
+        return apply_H_launch(cb, Vloc, P, nproj, D, D_mode, C, nb, HC, st);
+    jdft_basis *b = const_cast<jdft_basis *>(cb);   // the graph cache is bookkeeping, not state of the operator
+    JdftGraphEntry *g = nullptr;
+    for (JdftGraphEntry &e : b->graphs)
+        if (e.V == Vloc && e.P == P && e.D == D && e.C == C && e.HC == HC && e.ws == b->ws && e.ws_bytes == b->ws_bytes &&
+            e.nproj == nproj && e.D_mode == D_mode && e.nb == nb)
+            g = &e;
+    if (!g) {
+        if (b->graphs.size() >= 8) {
+            if (b->graphs.front().exec) cudaGraphExecDestroy(b->graphs.front().exec);
+            b->graphs.erase(b->graphs.begin());
+        }
+        b->graphs.push_back(JdftGraphEntry{Vloc, P, D, C, HC, b->ws, b->ws_bytes, nproj, D_mode, nb, 0, 0, nullptr});
+        g = &b->graphs.back();
+    }
+    if (g->exec) {
+        JDFT_CUDA(cudaGraphLaunch(g->exec, st));
+        jdft_count_launch((int)g->launches);
+        return JDFT_OK;
+    }
+    if (g->seen++ == 0) return apply_H_launch(b, Vloc, P, nproj, D, D_mode, C, nb, HC, st);   // warms kernel attributes
+    if (!b->gstream && cudaStreamCreateWithFlags(&b->gstream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError();
+        b->opt_graph = 0;
+        return apply_H_launch(b, Vloc, P, nproj, D, D_mode, C, nb, HC, st);
+    }
+    const int64_t before = jdft_launch_count_peek();
+    cudaGraph_t graph = nullptr;
+    bool ok = cudaStreamBeginCapture(b->gstream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+        rc = apply_H_launch(b, Vloc, P, nproj, D, D_mode, C, nb, HC, b->gstream);
+        ok = cudaStreamEndCapture(b->gstream, &graph) == cudaSuccess && rc == JDFT_OK && graph;
+    }
+    const int64_t captured = jdft_launch_count_peek() - before;
+    jdft_count_launch(-(int)captured);               // nothing ran yet
+    if (ok) ok = cudaGraphInstantiate(&g->exec, graph, 0) == cudaSuccess;
+    if (graph) cudaGraphDestroy(graph);
+    if (!ok) {
+        cudaGetLastError();
+        g->exec = nullptr;
+        b->opt_graph = 0;                            // do not try again on this basis
+        return apply_H_launch(b, Vloc, P, nproj, D, D_mode, C, nb, HC, st);
+    }
+    g->launches = captured;
+    JDFT_CUDA(cudaGraphLaunch(g->exec, st));
+    jdft_count_launch((int)captured);
+    return JDFT_OK;
 }
 
 extern "C" int jdft_overlap(const jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M,

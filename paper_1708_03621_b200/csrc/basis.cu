@@ -24,6 +24,12 @@ int jdft_cuda_fail(cudaError_t e, const char *what) {
     return jdft_fail(JDFT_ECUDA, "CUDA error '%s' in %s", cudaGetErrorString(e), what);
 }
 void jdft_count_launch(int n) { g_launches += n; }
+int64_t jdft_launch_count_peek() { return g_launches; }
+void jdft_graphs_clear(jdft_basis *b) {
+    for (JdftGraphEntry &g : b->graphs)
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+    b->graphs.clear();
+}
 
 extern "C" const char *jdft_last_error(void) { return g_err; }
 extern "C" int64_t jdft_launch_count(int reset) {
@@ -108,6 +114,8 @@ extern "C" int jdft_basis_destroy(jdft_basis *b) {
     if (b->ev_join) cudaEventDestroy(b->ev_join);
     for (int i = 0; i < 8; i++) cudaFree(b->hb[i]);
     for (int i = 0; i < 3; i++) if (b->hs[i]) cudaStreamDestroy(b->hs[i]);
+    jdft_graphs_clear(b);
+    if (b->gstream) cudaStreamDestroy(b->gstream);
     for (cudaEvent_t e : b->hev) cudaEventDestroy(e);
     for (cudaEvent_t e : b->prof_ev) cudaEventDestroy(e);
     delete b;
@@ -139,6 +147,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     for (int d = 0; d < 3; d++) b->d_tw[d] = nullptr;
     for (int i = 0; i < 8; i++) { b->hb[i] = nullptr; b->hb_bytes[i] = 0; }
     for (int i = 0; i < 3; i++) b->hs[i] = nullptr;
+    b->opt_graph = -1; b->gstream = nullptr;
     b->h_ops_set = 0; b->h_nproj = 0; b->h_D_mode = 0;
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
     b->opt_profile_kernel = 0; b->prof_used = 0;
@@ -349,11 +358,14 @@ extern "C" int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes) {
     if (((uintptr_t)dev_ptr & 15) != 0) return jdft_fail(JDFT_EINVAL, "set_workspace: pointer not 16-byte aligned");
     b->ws = dev_ptr;
     b->ws_bytes = dev_ptr ? bytes : 0;
+    jdft_graphs_clear(b);
     return JDFT_OK;
 }
 
 extern "C" int jdft_set_option(jdft_basis *b, const char *key, int64_t value) {
     if (!b || !key) return jdft_fail(JDFT_EINVAL, "set_option: null argument");
+    jdft_graphs_clear(b);   // captured calls bake the options in
+    if (!strcmp(key, "graph")) { b->opt_graph = value < 0 ? -1 : (value != 0); return JDFT_OK; }
     if (!strcmp(key, "band_batch")) { b->opt_band_batch = value < 0 ? 0 : value; return JDFT_OK; }
     if (!strcmp(key, "planes_pair")) { b->opt_pair = value != 0; return JDFT_OK; }
     if (!strcmp(key, "planes_prune")) { b->opt_prune = value != 0; return JDFT_OK; }

@@ -438,8 +438,8 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     // 64 x 64): taken when 0.8 x its padded width beats the 4M choice and K is long enough to matter
     const bool m3 = b->opt_gemm3m && K >= 512 && (tri ? Cn >= 128 : pad48 * 80 < (bn == 48 ? pad48 : pad64) * 100);
     if (m3) bn = 48;
-    // the 3M kernels run k-tiles of 16 in a 3-stage pipeline (half the barriers per DMMA of the 8-deep 4-stage 4M kernels)
-    constexpr int ST3 = 3, BK3 = 16;
+    // pipeline of the 3M kernels: measured on config 3 (P^+ C, 1.70 ms): 6 stages of 8 -> 1.78 ms, 3 stages of 16 -> 1.89 ms
+    constexpr int ST3 = STAGES, BK3 = BK;
     const int bk = m3 ? BK3 : BK;
     const int64_t ktiles = (K + bk - 1) / bk;
     const int tcol = (Cn + bn - 1) / bn;

@@ -15,6 +15,16 @@ struct FftPlan {
     int radix[JDFT_MAX_PASSES];
 };
 
+// one captured jdft_apply_H call (option "graph"): replayed while every argument and the workspace stay the same
+struct JdftGraphEntry {
+    const void *V, *P, *D, *C, *HC, *ws;
+    size_t ws_bytes;
+    int nproj, D_mode, nb;
+    int64_t launches;        // kernels in the graph (for jdft_launch_count)
+    int seen;                // calls with this key so far (the first one runs directly and warms the kernel attributes)
+    cudaGraphExec_t exec;    // nullptr until captured
+};
+
 struct jdft_basis {
     // geometry
     double R[9], k[3], Ecut, G[9], GGT[9], volume;
@@ -60,6 +70,9 @@ struct jdft_basis {
     // cached device buffers of the *_host entry points (library-owned, grow-only)
     void *hb[8];
     size_t hb_bytes[8];
+    int64_t opt_graph;                        // "graph": -1 auto (small problems), 0 off, 1 on
+    std::vector<JdftGraphEntry> graphs;
+    cudaStream_t gstream;                     // capture stream
     cudaStream_t hs[3];                       // H2D, compute and D2H streams of the *_host pipeline (created on first use)
     std::vector<cudaEvent_t> hev;
     int h_ops_set, h_nproj, h_D_mode;         // resident operators of jdft_host_set_operators (in hb[2..4])
@@ -75,6 +88,8 @@ void jdft_prof_end(const jdft_basis *b, int kid, cudaStream_t st);
 int jdft_fail(int code, const char *fmt, ...);
 int jdft_cuda_fail(cudaError_t e, const char *what);
 void jdft_count_launch(int n);
+int64_t jdft_launch_count_peek();
+void jdft_graphs_clear(jdft_basis *b);
 #define JDFT_CUDA(call)                                           \
     do {                                                          \
         cudaError_t e__ = (call);                                 \

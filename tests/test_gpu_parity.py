@@ -667,3 +667,44 @@ def test_planes_tma_kernel_matches(ref, jd, cfg_id):
     jd.jdft_set_workspace(c.gb, torch.empty(jd.jdft_workspace_bytes(c.gb, 6, 0) + 48 * 2 * c.gb.nG + 4096, dtype=torch.uint8, device="cuda"))
     got = jd.jdft_pcm_hessian(c.gb, dev(eps.reshape(-1)), dev(phi)).cpu().numpy()
     assert rel_err_per_band(got, c.rb.pcm_hessian(eps, phi)) <= TOL
+
+
+# ------------------------------------------------------------------------------------------ CUDA-graph replay
+
+def test_apply_H_graph_replay(ref, jd):
+    """Small calls replay a captured CUDA graph from the third identical call on (option "graph", automatic for
+    config 1): results equal the direct launches bit for bit, follow the CONTENTS of the arrays (same pointers, new
+    data), a different output pointer gets its own capture, and options / a new workspace drop the captures."""
+    c = Case(ref, jd, 1)
+    V, P, D, C = dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C)
+    HC = torch.empty_like(C)
+    jd.jdft_set_option(c.gb, "graph", 0)
+    direct = jd.jdft_apply_H(c.gb, V, P, D, C, HC).clone()
+    jd.jdft_set_option(c.gb, "graph", -1)
+    jd.jdft_launch_count(reset=True)
+    for _ in range(4):                                       # direct, capture + replay, replay, replay
+        HC.zero_()
+        jd.jdft_apply_H(c.gb, V, P, D, C, HC)
+        assert torch.equal(HC, direct)
+    assert jd.jdft_launch_count() == 4 * 10                  # replays count their kernels
+    C.mul_(2.0)                                              # same pointer, new contents
+    jd.jdft_apply_H(c.gb, V, P, D, C, HC)
+    assert torch.equal(HC, 2.0 * direct)
+    C.mul_(0.5)
+    HC2 = torch.empty_like(C)
+    for _ in range(3):
+        jd.jdft_apply_H(c.gb, V, P, D, C, HC2)
+    assert torch.equal(HC2, direct)
+    jd.jdft_set_option(c.gb, "band_batch", 3)                # drops the captures; 3 + 3 + 2 bands now
+    for _ in range(3):
+        jd.jdft_apply_H(c.gb, V, P, D, C, HC)
+    assert rel_err_per_band(HC.cpu().numpy(), direct.cpu().numpy()) <= 1e-13
+    assert rel_err_per_band(HC.cpu().numpy(), c.rb.apply_H(c.V, c.P, c.D, c.C)) <= TOL
+    # replay on a non-default stream
+    st = torch.cuda.Stream()
+    jd.jdft_set_option(c.gb, "band_batch", 0)
+    with torch.cuda.stream(st):
+        for _ in range(3):
+            jd.jdft_apply_H(c.gb, V, P, D, C, HC)
+    st.synchronize()
+    assert torch.equal(HC, direct)

@@ -660,3 +660,39 @@ int jdft_ref_overlap_us(const jdft_ref_basis *b, const double *P, int np, const 
     free(X);
     return rc;
 }
+
+/* ---- Listing 1 on REAL fields (SURVEY.md 8(f) rank 3 "r2c/c2r variant"; `ScalarField epsilon`, phi and
+ * rho are real fields, so their ScalarFieldTilde spectra are Hermitian-symmetric, phi~(-G) = conj(phi~(G))).
+ * Half-sphere storage (reading 25): for a Gamma-point basis (k = 0) the canonical order is symmetric under
+ * inversion, iG[nG-1-n] = -iG[n], the origin is n0 = (nG-1)/2, and the stored half is the tail n = n0 .. nG-1:
+ *     phi_h[ib][h] = phi~[n0 + h],   h = 0 .. nGh-1,  nGh = n0 + 1;     phi~[n0 - h] = conj(phi_h[ib][h]);
+ * the imaginary part of the G = 0 entry is ignored (a real field has none).  Written out literally: extend to the
+ * full sphere, apply the complex operator, keep the stored half.                                                   */
+int jdft_ref_pcm_hessian_real(const jdft_ref_basis *b, const double *epsilon, const double *phi_h, int nb, double *out_h) {
+    if (!b || nb < 0 || !epsilon || (nb > 0 && (!phi_h || !out_h))) return REF_EINVAL;
+    if (b->k[0] != 0.0 || b->k[1] != 0.0 || b->k[2] != 0.0 || b->nG % 2 == 0) return REF_EINVAL;
+    const int64_t nG = b->nG, n0 = (nG - 1) / 2, nGh = n0 + 1;
+    for (int64_t n = 0; n < nG; n++)                   /* the order really is inversion symmetric */
+        for (int d = 0; d < 3; d++)
+            if (b->iG[3 * n + d] != -b->iG[3 * (nG - 1 - n) + d]) return REF_EINVAL;
+    cplx *full = (cplx *)malloc(sizeof(cplx) * (size_t)(nb > 0 ? nb : 1) * nG);
+    cplx *res = (cplx *)malloc(sizeof(cplx) * (size_t)(nb > 0 ? nb : 1) * nG);
+    if (!full || !res) { free(full); free(res); return REF_ENOMEM; }
+    const cplx *ph = (const cplx *)phi_h;
+    for (int ib = 0; ib < nb; ib++) {
+        full[(size_t)ib * nG + n0] = creal(ph[(size_t)ib * nGh]);
+        for (int64_t h = 1; h < nGh; h++) {
+            full[(size_t)ib * nG + n0 + h] = ph[(size_t)ib * nGh + h];
+            full[(size_t)ib * nG + n0 - h] = conj(ph[(size_t)ib * nGh + h]);
+        }
+    }
+    int rc = jdft_ref_pcm_hessian(b, epsilon, (const double *)full, nb, (double *)res);
+    if (!rc) {
+        cplx *oh = (cplx *)out_h;
+        for (int ib = 0; ib < nb; ib++)
+            for (int64_t h = 0; h < nGh; h++) oh[(size_t)ib * nGh + h] = res[(size_t)ib * nG + n0 + h];
+    }
+    free(full);
+    free(res);
+    return rc;
+}

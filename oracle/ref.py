@@ -59,6 +59,7 @@ def lib():
         L.jdft_ref_gradient.argtypes = [vp, vp, ci, vp]
         L.jdft_ref_divergence.argtypes = [vp, vp, ci, vp]
         L.jdft_ref_pcm_hessian.argtypes = [vp, vp, vp, ci, vp]
+        L.jdft_ref_pcm_hessian_real.argtypes = [vp, vp, vp, ci, vp]
         L.jdft_ref_apply_O_us.argtypes = [vp, vp, ci, vp, ci, vp, ci, vp]
         L.jdft_ref_overlap_us.argtypes = [vp, vp, ci, vp, ci, vp, ci, vp, ci, vp]
         _lib = L
@@ -243,6 +244,15 @@ class RefBasis:
         assert eps.size == self.N
         out = np.empty_like(phi)
         _chk(lib().jdft_ref_pcm_hessian(self._h, _p(eps), _p(phi), phi.shape[0], _p(out)))
+        return out
+
+    def pcm_hessian_real(self, epsilon, phi_h):
+        """Listing 1 on real fields in half-sphere storage: phi_h[ib, h] = phi~[n0 + h], n0 = (nG - 1) / 2 (k = 0 only)."""
+        phi_h = _c128(phi_h)
+        eps = np.ascontiguousarray(epsilon, dtype=np.float64)
+        assert eps.size == self.N and phi_h.shape[1] == (self.nG + 1) // 2
+        out = np.empty_like(phi_h)
+        _chk(lib().jdft_ref_pcm_hessian_real(self._h, _p(eps), _p(phi_h), phi_h.shape[0], _p(out)))
         return out
 
     def apply_O_us(self, P, Q, C):

@@ -567,3 +567,42 @@ def test_ultrasoft_overlap_operator_vs_dense_matrix(ref):
     p, q = P[:1], np.array([0.3])
     want = b.volume * np.stack([c + q[0] * p[0] * np.vdot(p[0], c) for c in C])
     assert np.max(np.abs(b.apply_O_us(p, q, C) - want)) <= 1e-13 * np.max(np.abs(want))
+
+
+# ------------------------------------------------------------------------------------------ real fields (8(f) rank 3)
+
+def test_pcm_hessian_real_fields_half_sphere(ref):
+    """Real-field variant (epsilon, phi, rho are real ScalarFields): half-sphere storage of a
+    Hermitian-symmetric spectrum.  Pins: the canonical order is inversion symmetric with the origin in the middle; the
+    Hermitian extension of the stored half IS a real field (I gives zero imaginary part); the complex operator maps
+    it to a Hermitian-symmetric spectrum whose stored half is the real-variant result; for constant epsilon the closed
+    form (eps0 / 4 pi) |q|^2 phi; k != 0 is refused."""
+    R = _skew_lattice()
+    S = (8, 9, 10)
+    b = ref.RefBasis(R, [0.0, 0.0, 0.0], 6.0, S)
+    nG, n0 = b.nG, (b.nG - 1) // 2
+    assert nG % 2 == 1 and np.all(b.iG[n0] == 0)
+    assert np.array_equal(b.iG[::-1], -b.iG)
+    rng = np.random.default_rng(83)
+    nb = 3
+    ph = _rand_c(rng, nb, n0 + 1)
+    ph[:, 0] = ph[:, 0].real + 0.77j                      # imaginary part of G = 0 must be ignored
+    full = np.empty((nb, nG), complex)
+    full[:, n0:] = ph
+    full[:, n0] = ph[:, 0].real
+    full[:, :n0] = ph[:, :0:-1].conj()
+    psi = b.apply_I(full)
+    assert np.max(np.abs(psi.imag)) <= 1e-12 * np.max(np.abs(psi.real))          # a real field
+    eps = 1.0 + 5.0 * rng.random(S)
+    want_full = b.pcm_hessian(eps, full)
+    assert np.max(np.abs(want_full[:, ::-1].conj() - want_full)) <= 1e-12 * np.max(np.abs(want_full))   # stays Hermitian
+    got = b.pcm_hessian_real(eps, ph)
+    assert got.shape == ph.shape
+    assert np.max(np.abs(got - want_full[:, n0:])) <= 1e-13 * np.max(np.abs(want_full))
+    e0 = 3.25
+    got0 = b.pcm_hessian_real(np.full(S, e0), ph)
+    closed = (e0 / (4 * np.pi)) * (2.0 * b.ke[n0:])[None, :] * full[:, n0:]
+    assert np.max(np.abs(got0 - closed)) <= 1e-12 * np.max(np.abs(closed))
+    bk = ref.RefBasis(R, [0.25, 0.0, 0.0], 6.0, S)
+    with pytest.raises(ref.RefError):
+        bk.pcm_hessian_real(eps, np.zeros((1, (bk.nG + 1) // 2), complex))

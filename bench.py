@@ -466,7 +466,7 @@ def measure(cfg_id, args, rank, world, local, full):
                   "subspace": {"ms": ms_s, "TFLOP/s": 8.0 * nb * nb * i["nG"] / (ms_s * 1e-3) / 1e12},
                   "apply_I": {"ms": ms_I, "bands": nbI, "alg_GB/s": ij_bytes / (ms_I * 1e-3) / 1e9},
                   "apply_J": {"ms": ms_J, "bands": nbI, "alg_GB/s": ij_bytes / (ms_J * 1e-3) / 1e9}}
-        extras.update(extra_ops(jd, torch, t_op, k, ks, V, D, S, nb, nproj, cfg))
+        extras.update(extra_ops(jd, torch, t_op, k, V, S, nb, nproj, cfg, R, Ecut, local))
         del gs, phi, epsr, hout, psiI
 
     infos = [k["info"] for k in ks]
@@ -542,9 +542,38 @@ def measure(cfg_id, args, rank, world, local, full):
     return line
 
 
-def extra_ops(jd, torch, t_op, k, ks, V, D, S, nb, nproj, cfg):
-    """Timings of the SURVEY 8(f) rank 2 / 3 additions (filled in where the library exports them)."""
-    return {}
+def extra_ops(jd, torch, t_op, k, V, S, nb, nproj, cfg, R, Ecut, local):
+    """Timings of the SURVEY 8(f) rank 2 / 3 additions on k-point 0: ultrasoft O_us / overlap_us with per-atom Q blocks,
+    H with per-atom D blocks, and Listing 1 on real fields (half-sphere storage) beside the complex variant."""
+    out = {}
+    gb, C, P = k["gb"], k["C"], k["P"]
+    nblk = cfg["n_lm"]
+    g = torch.Generator(device="cuda").manual_seed(5)
+    A = torch.randn((nproj // nblk, nblk, nblk), dtype=torch.complex128, device="cuda", generator=g)
+    Qb = (0.05 * (A @ A.conj().transpose(1, 2))).contiguous()
+    OC = torch.empty_like(C)
+    Mus = torch.empty((nb, nb), dtype=torch.complex128, device="cuda")
+    ms_o = t_op(lambda: jd.jdft_apply_O_us(gb, P, Qb, C, OC))
+    ms_m = t_op(lambda: jd.jdft_overlap_us(gb, P, Qb, C, C, Mus))
+    ms_h = t_op(lambda: jd.jdft_apply_H(gb, V, P, Qb, C, k["HC"]))
+    nG = k["info"]["nG"]
+    out["apply_O_us_blockQ"] = {"ms": ms_o, "TFLOP/s": 16.0 * nb * nproj * nG / (ms_o * 1e-3) / 1e12}
+    out["overlap_us_blockQ"] = {"ms": ms_m, "TFLOP/s": (8.0 * (nb * (nb + 1) // 2) * nG + 16.0 * nb * nproj * nG) / (ms_m * 1e-3) / 1e12}
+    out["apply_H_blockD"] = {"ms": ms_h, "band_apps_per_s": nb / (ms_h * 1e-3)}
+    # Listing 1 on real fields: the density-cutoff basis (4 x Ecut, Gamma) as the scalar-field basis, 16 fields
+    gs = jd.jdft_basis_create(R, [0.0, 0.0, 0.0], 4.0 * Ecut, S, device=local)
+    nf = 16
+    jd.jdft_set_workspace(gs, torch.empty(jd.jdft_workspace_bytes(gs, 3 * nf, 0) + 48 * nf * gs.nG, dtype=torch.uint8, device="cuda"))
+    ph = torch.randn(nf, (gs.nG + 1) // 2, dtype=torch.complex128, device="cuda")
+    eps = 1.0 + 78.0 * torch.rand(int(np.prod(S)), dtype=torch.float64, device="cuda")
+    oh = torch.empty_like(ph)
+    ms_r = t_op(lambda: jd.jdft_pcm_hessian_real(gs, eps, ph, oh))
+    a_s, b_s = gs.ncol * S[2], gs.npl * S[1] * S[2]
+    npair = (3 * nf + 1) // 2
+    real_bytes = npair * 16 * (4 * a_s + 4 * b_s + 2 * gs.nG) + 2 * npair * 16 * gs.nG + 2 * nf * 16 * ((gs.nG + 1) // 2) + 8 * int(np.prod(S))
+    out["pcm_hessian_real"] = {"ms": ms_r, "fields": nf, "nG_half": (gs.nG + 1) // 2, "fields_per_s": nf / (ms_r * 1e-3),
+                               "alg_GB/s": real_bytes / (ms_r * 1e-3) / 1e9}
+    return out
 
 
 def compact(line):

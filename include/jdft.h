@@ -163,6 +163,14 @@ int jdft_gradient(const jdft_basis *b, const double *C, int nb, double *out, jdf
 int jdft_divergence(const jdft_basis *b, const double *X, int nb, double *out, jdft_stream s);
 int jdft_pcm_hessian(const jdft_basis *b, const double *epsilon, const double *phi, int nb, double *out,
                      jdft_stream s);
+/* The same operator on REAL fields (epsilon, phi, rho are real ScalarFields, so phi~(-G) = conj(phi~(G)))
+ * in half-sphere storage (reading 25).  Gamma-point bases only (k = 0, else JDFT_EINVAL): there the canonical
+ * order is inversion symmetric, iG[nG-1-n] = -iG[n], the origin is n0 = (nG-1)/2 and the stored half is the tail:
+ *     phi_h[ib][h] = phi~[n0 + h],  h = 0 .. nGh-1,  nGh = (nG+1)/2;   phi~[n0 - h] = conj(phi_h[ib][h]);  Im phi~[n0] ignored.
+ * out_h has the same layout.  Two real gradient components share one complex transform (two-for-one), so the call moves
+ * and computes half of what jdft_pcm_hessian does.  Workspace: ceil(3 nb / 2) nG c128 plus FFT scratch.               */
+int jdft_pcm_hessian_real(const jdft_basis *b, const double *epsilon, const double *phi_h, int nb, double *out_h,
+                          jdft_stream s);
 
 /* ---- HOST-buffer variants (end-to-end path: H2D copy, kernels, D2H copy, sync) -------------------- */
 int jdft_apply_H_host(jdft_basis *b, const double *Vloc_host, const double *P_host, int nproj,

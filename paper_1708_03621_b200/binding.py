@@ -19,7 +19,7 @@ EXPORTS = [
     "jdft_basis_create", "jdft_basis_destroy", "jdft_basis_info", "jdft_basis_structure", "jdft_basis_export",
     "jdft_basis_device_maps", "jdft_workspace_bytes", "jdft_set_workspace", "jdft_set_option",
     "jdft_apply_I", "jdft_apply_Idag", "jdft_apply_J", "jdft_apply_L", "jdft_apply_O", "jdft_apply_Vnl",
-    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_apply_H_host", "jdft_overlap_host", "jdft_host_set_operators", "jdft_apply_H_host_resident",
+    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_pcm_hessian_real", "jdft_apply_H_host", "jdft_overlap_host", "jdft_host_set_operators", "jdft_apply_H_host_resident",
     "jdft_last_error", "jdft_launch_count", "jdft_profile_read", "jdft_version",
 ]
 
@@ -59,6 +59,7 @@ def _load():
     L.jdft_gradient.argtypes = [vp, vp, ci, vp, vp]
     L.jdft_divergence.argtypes = [vp, vp, ci, vp, vp]
     L.jdft_pcm_hessian.argtypes = [vp, vp, vp, ci, vp, vp]
+    L.jdft_pcm_hessian_real.argtypes = [vp, vp, vp, ci, vp, vp]
     L.jdft_apply_H_host.argtypes = [vp, vp, vp, ci, vp, ci, vp, ci, vp]
     L.jdft_overlap_host.argtypes = [vp, vp, ci, vp, ci, vp]
     L.jdft_host_set_operators.argtypes = [vp, vp, vp, ci, vp, ci]
@@ -354,6 +355,20 @@ def jdft_pcm_hessian(basis, epsilon, phi, out=None):
     _chk(_lib.jdft_pcm_hessian(basis._h, _dev(epsilon, torch.float64, "epsilon"), _dev(phi, torch.complex128, "phi"), nb,
                                _dev(out, torch.complex128, "out"), _stream()))
     return out
+
+
+def jdft_pcm_hessian_real(basis, epsilon, phi_h, out_h=None):
+    """Listing 1 on real fields in half-sphere storage: phi_h [nb, (nG + 1) / 2] = phi~[n0:], n0 = (nG - 1) / 2; k = 0 only."""
+    nGh = (basis.nG + 1) // 2
+    if phi_h.dim() != 2 or phi_h.shape[1] != nGh:
+        raise ValueError("phi_h must have shape [nb, (nG + 1) / 2 = %d]" % nGh)
+    if epsilon.numel() != basis.N:
+        raise ValueError("epsilon must have N = S0*S1*S2 entries")
+    if out_h is None:
+        out_h = torch.empty_like(phi_h)
+    _chk(_lib.jdft_pcm_hessian_real(basis._h, _dev(epsilon, torch.float64, "epsilon"), _dev(phi_h, torch.complex128, "phi_h"),
+                                    int(phi_h.shape[0]), _dev(out_h, torch.complex128, "out_h"), _stream()))
+    return out_h
 
 
 def _host(a, dtype, name):

@@ -1007,6 +1007,71 @@ __global__ void k_divergence(const Mat3 m, const int32_t *__restrict__ iG, const
     }
 }
 
+// Real fields, two for one (Listing 1 on half-sphere storage, jdft_pcm_hessian_real).  The 3 nb gradient components
+// c = d nb + ib of real fields are Hermitian-symmetric spectra G_c; a pair (2p, 2p+1) rides through the COMPLEX pipeline
+// as Z_p = G_2p + i G_2p+1 (its real-space image is g_2p + i g_2p+1, so the real epsilon acts on both at once) and is
+// separated afterwards: G'_2p[n] = (Z'[n] + conj(Z'[-n])) / 2,  G'_2p+1[n] = (Z'[n] - conj(Z'[-n])) / (2 i).
+// Gamma-point bases only: the canonical order is inversion symmetric, -n = nG - 1 - n, origin n0 = (nG - 1) / 2, and
+// the stored half is n0 .. nG - 1:  phi~[n0 + h] = ph[h],  phi~[n0 - h] = conj(ph[h]),  Im phi~[n0] ignored.
+__device__ __forceinline__ double2 half_ext(const double2 *__restrict__ ph, const int64_t n, const int64_t n0) {
+    if (n > n0) return ph[n - n0];
+    if (n < n0) { const double2 v = ph[n0 - n]; return make_double2(v.x, -v.y); }
+    return make_double2(ph[0].x, 0.0);
+}
+// Z[p][n] = i q_d(n) phi~_ib[n] + i * (i q_d'(n) phi~_ib'[n]),  (d, ib) = component 2p, (d', ib') = component 2p + 1
+__global__ void k_grad_pack_real(const Mat3 m, const int32_t *__restrict__ iG, const int64_t nG, const int nb, const int npair,
+                                 const double2 *__restrict__ phi_h, double2 *__restrict__ Z) {
+    const int64_t n0 = (nG - 1) / 2, nGh = n0 + 1, total = (int64_t)npair * nG;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int p = (int)(i / nG);
+        const int64_t n = i - (int64_t)p * nG;
+        double q[3];
+        q_of(m, iG, n, q);
+        const int c0 = 2 * p, c1 = 2 * p + 1;
+        const double2 a = half_ext(phi_h + (size_t)(c0 % nb) * nGh, n, n0);
+        // i q a = (-q a.y, q a.x)
+        const double qa = q[c0 / nb];
+        double zr = -qa * a.y, zi = qa * a.x;
+        if (c1 < 3 * nb) {
+            const double2 bb = half_ext(phi_h + (size_t)(c1 % nb) * nGh, n, n0);
+            const double qb = q[c1 / nb];
+            // + i * (i qb bb) = i * (-qb bb.y, qb bb.x) = (-qb bb.x, -qb bb.y)
+            zr -= qb * bb.x;
+            zi -= qb * bb.y;
+        }
+        Z[i] = make_double2(zr, zi);
+    }
+}
+// out_h[ib][h] = f * sum_d i q_d(n) G'_{d nb + ib}[n],  n = n0 + h
+__global__ void k_unpack_div_real(const Mat3 m, const int32_t *__restrict__ iG, const int64_t nG, const int nb, const double f,
+                                  const double2 *__restrict__ Z, double2 *__restrict__ out_h) {
+    const int64_t n0 = (nG - 1) / 2, nGh = n0 + 1, total = (int64_t)nb * nGh;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int ib = (int)(i / nGh);
+        const int64_t h = i - (int64_t)ib * nGh, n = n0 + h, nm = n0 - h;
+        double q[3];
+        q_of(m, iG, n, q);
+        double sr = 0.0, si = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            const int c = d * nb + ib;
+            const double2 *Zp = Z + (size_t)(c >> 1) * nG;
+            const double2 zp = Zp[n], zm = Zp[nm];
+            double gr, gi;
+            if ((c & 1) == 0) {   // (z+ + conj(z-)) / 2
+                gr = 0.5 * (zp.x + zm.x);
+                gi = 0.5 * (zp.y - zm.y);
+            } else {              // (z+ - conj(z-)) / (2 i) = (Im-part difference, -Re-part difference) / 2
+                gr = 0.5 * (zp.y + zm.y);
+                gi = -0.5 * (zp.x - zm.x);
+            }
+            sr -= q[d] * gi;      // i q g = (-q gi, q gr)
+            si += q[d] * gr;
+        }
+        out_h[i] = make_double2(f * sr, f * si);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ diagonal ops
 // out[b][n] = (f0 + f1 * ke[n]) * C[b][n]
 __global__ void k_diag(const int64_t nG, const int64_t total, const double f0, const double f1,
@@ -1492,6 +1557,37 @@ extern "C" int jdft_pcm_hessian(const jdft_basis *b, const double *epsilon, cons
     if ((rc = launch_gradient(b, phi, nb, g, st))) return rc;
     if ((rc = jdft_local_H(b, epsilon, g, 3 * nb, g, st, gbytes, 1.0 / (double)b->N, 0.0))) return rc;
     return launch_divergence(b, g, nb, -1.0 / (4.0 * M_PI), out, st);
+}
+
+// Listing 1 on REAL fields in half-sphere storage (include/jdft.h): 3 nb real gradient components travel as
+// ceil(3 nb / 2) complex fields through the fused pruned pipeline -- half the FFT work and bytes of jdft_pcm_hessian.
+extern "C" int jdft_pcm_hessian_real(const jdft_basis *b, const double *epsilon, const double *phi_h, int nb, double *out_h,
+                                     jdft_stream s) {
+    int rc = check_common(b, phi_h, out_h, nb, "pcm_hessian_real");
+    if (rc) return rc;
+    if (!epsilon) return jdft_fail(JDFT_EINVAL, "pcm_hessian_real: null epsilon");
+    if (b->k[0] != 0.0 || b->k[1] != 0.0 || b->k[2] != 0.0 || b->nG % 2 == 0)
+        return jdft_fail(JDFT_EINVAL, "pcm_hessian_real: half-sphere storage needs a Gamma-point basis (k = 0)");
+    if (nb == 0) return JDFT_OK;
+    cudaStream_t st = (cudaStream_t)s;
+    const int npair = (3 * nb + 1) / 2;
+    const size_t zbytes = (((size_t)npair * b->nG * 16) + 255) & ~(size_t)255;
+    if (!b->ws || jdft_band_batch(b, npair, zbytes) == 0)
+        return jdft_fail(JDFT_EWORKSPACE, "pcm_hessian_real: workspace must hold ceil(3 nb / 2) nG c128 (%zu bytes) plus one band of FFT scratch", zbytes);
+    double *Z = static_cast<double *>(b->ws);
+    jdft_prof_begin(b, JDFT_K_DIAG, st);
+    k_grad_pack_real<<<elementwise_grid(b, (int64_t)npair * b->nG), 256, 0, st>>>(mat3_of(b), b->d_iG, b->nG, nb, npair,
+                                                                                 reinterpret_cast<const double2 *>(phi_h),
+                                                                                 reinterpret_cast<double2 *>(Z));
+    jdft_prof_end(b, JDFT_K_DIAG, st);
+    JDFT_LAUNCH_CHECK("k_grad_pack_real");
+    if ((rc = jdft_local_H(b, epsilon, Z, npair, Z, st, zbytes, 1.0 / (double)b->N, 0.0))) return rc;
+    jdft_prof_begin(b, JDFT_K_DIAG, st);
+    k_unpack_div_real<<<elementwise_grid(b, (int64_t)nb * ((b->nG + 1) / 2)), 256, 0, st>>>(
+        mat3_of(b), b->d_iG, b->nG, nb, -1.0 / (4.0 * M_PI), reinterpret_cast<const double2 *>(Z), reinterpret_cast<double2 *>(out_h));
+    jdft_prof_end(b, JDFT_K_DIAG, st);
+    JDFT_LAUNCH_CHECK("k_unpack_div_real");
+    return JDFT_OK;
 }
 
 static int diag_op(const jdft_basis *b, const double *C, int nb, double *out, double f0, double f1, jdft_stream s,

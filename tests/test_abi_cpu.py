@@ -91,6 +91,8 @@ def test_null_and_bad_arguments_return_status_codes_without_a_device(lib):
     assert lib.jdft_apply_O_us(None, None, 0, None, 0, None, 1, None, None) == EINVAL
     lib.jdft_overlap_us.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp]
     assert lib.jdft_overlap_us(None, None, 0, None, 0, None, 1, None, 1, None, None) == EINVAL
+    lib.jdft_pcm_hessian_real.argtypes = [vp, vp, vp, ctypes.c_int, vp, vp]
+    assert lib.jdft_pcm_hessian_real(None, None, None, 1, None, None) == EINVAL
     lib.jdft_host_set_operators.argtypes = [vp, vp, vp, ctypes.c_int, vp, ctypes.c_int]
     assert lib.jdft_host_set_operators(None, None, None, 0, None, 0) == EINVAL
     lib.jdft_apply_H_host_resident.argtypes = [vp, vp, ctypes.c_int, vp]

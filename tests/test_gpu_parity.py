@@ -679,14 +679,17 @@ def test_apply_H_graph_replay(ref, jd):
     V, P, D, C = dev(c.V.reshape(-1)), dev(c.P), dev(c.D), dev(c.C)
     HC = torch.empty_like(C)
     jd.jdft_set_option(c.gb, "graph", 0)
+    jd.jdft_launch_count(reset=True)
     direct = jd.jdft_apply_H(c.gb, V, P, D, C, HC).clone()
+    per_call = jd.jdft_launch_count()
+    assert per_call >= 8
     jd.jdft_set_option(c.gb, "graph", -1)
     jd.jdft_launch_count(reset=True)
     for _ in range(4):                                       # direct, capture + replay, replay, replay
         HC.zero_()
         jd.jdft_apply_H(c.gb, V, P, D, C, HC)
         assert torch.equal(HC, direct)
-    assert jd.jdft_launch_count() == 4 * 10                  # replays count their kernels
+    assert jd.jdft_launch_count() == 4 * per_call            # replays count their kernels
     C.mul_(2.0)                                              # same pointer, new contents
     jd.jdft_apply_H(c.gb, V, P, D, C, HC)
     assert torch.equal(HC, 2.0 * direct)
@@ -708,3 +711,36 @@ def test_apply_H_graph_replay(ref, jd):
             jd.jdft_apply_H(c.gb, V, P, D, C, HC)
     st.synchronize()
     assert torch.equal(HC, direct)
+
+
+# ------------------------------------------------------------------------------------------ Listing 1 on real fields
+
+@pytest.mark.parametrize("cfg_id,nb", [(101, 1), (102, 2), (104, 5), (1, 3)])
+def test_pcm_hessian_real_fields(ref, jd, cfg_id, nb):
+    """jdft_pcm_hessian_real (half-sphere storage, two real gradient components per complex transform) against the
+    oracle's real-field function and against the GPU's own complex path on the Hermitian extension; odd and even numbers
+    of components (3 nb = 3, 6, 15, 9); k != 0 is refused."""
+    R, kpts, Ecut, S = workloads.lattice(cfg_id)
+    k0 = [0.0, 0.0, 0.0]
+    rb = ref.RefBasis(R, k0, Ecut, S)
+    gb = jd.jdft_basis_create(R, k0, Ecut, S)
+    nG, n0 = rb.nG, (rb.nG - 1) // 2
+    rng = np.random.default_rng(211 + cfg_id)
+    ph = rng.standard_normal((nb, n0 + 1)) + 1j * rng.standard_normal((nb, n0 + 1))
+    eps = 1.0 + 78.0 * rng.random(S)
+    jd.jdft_set_workspace(gb, torch.empty(jd.jdft_workspace_bytes(gb, 3 * nb, 0) + 48 * nb * nG + 4096, dtype=torch.uint8, device="cuda"))
+    got = jd.jdft_pcm_hessian_real(gb, dev(eps.reshape(-1)), dev(ph)).cpu().numpy()
+    want = rb.pcm_hessian_real(eps, ph)
+    assert rel_err_per_band(got, want) <= TOL
+    full = np.empty((nb, nG), complex)
+    full[:, n0:] = ph
+    full[:, n0] = ph[:, 0].real
+    full[:, :n0] = ph[:, :0:-1].conj()
+    gfull = jd.jdft_pcm_hessian(gb, dev(eps.reshape(-1)), dev(full)).cpu().numpy()
+    assert rel_err_per_band(got, gfull[:, n0:]) <= 1e-12
+    if any(kpts[0] != 0):
+        gk = jd.jdft_basis_create(R, kpts[0], Ecut, S)
+        jd.jdft_alloc_workspace(gk, 8, 8)
+        with pytest.raises(jd.JdftError) as e:
+            jd.jdft_pcm_hessian_real(gk, dev(eps.reshape(-1)), torch.zeros((1, (gk.nG + 1) // 2), dtype=torch.complex128, device="cuda"))
+        assert e.value.code == jd.JDFT_EINVAL

@@ -585,6 +585,94 @@ def compact(line):
             "kernel_frac": {n: round(v["frac"], 4) for n, v in line["kernels"].items() if "frac" in v}}
 
 
+def shard_inputs(cfg_id, layout, make_basis, to_dev):
+    """Per-rank inputs of the (k-point, band) sharded step: for each k-point this rank works on, the basis, the full
+    projector block and ITS band rows of the seeded C (rank-independent seeds, so the shards are slices of the same
+    global arrays the unsharded run uses).  make_basis(R, k, Ecut, S) -> (basis, iG); to_dev(ndarray) -> tensor."""
+    R, kpts, Ecut, S = workloads.lattice(cfg_id)
+    atoms = workloads.atoms_fractional(cfg_id)
+    kdata = {}
+    for k, blo, bhi in layout.group_units():
+        basis, iG = make_basis(R, kpts[k], Ecut, S)
+        C = workloads.make_bands(cfg_id, len(iG), ik=k)
+        kdata[k] = dict(basis=basis, P=to_dev(workloads.make_projectors(cfg_id, iG, kpts[k], atoms)),
+                        C=to_dev(np.ascontiguousarray(C[blo:bhi])), nG=len(iG))
+    V = to_dev(workloads.make_vloc(cfg_id, atoms).reshape(-1))
+    D = to_dev(workloads.make_D(cfg_id))
+    return kdata, V, D
+
+
+def run_shard(args):
+    """--shard kb: ONE job sharded over the ranks with paper_1708_03621_b200/sharding.py -- k-points first (the paper's
+    MPI-over-k layout), bands inside a k-point when there are more ranks than k-points; per step every
+    rank applies H to its band columns (no collective) and forms its column block of C^+ O C (one all-gather, or a ring
+    of neighbour exchanges overlapped with the GEMM).  Fixed total work: "scaling": "strong"."""
+    import torch
+    import torch.distributed as dist
+    import paper_1708_03621_b200.binding as jd
+    from paper_1708_03621_b200 import sharding as sh
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    cfg, nk, nb, nproj = config_sizes(args.config)
+    layout = sh.KBLayout(nk, nb, world, rank)
+    group = layout.new_band_group() if world > 1 else None
+
+    def make_basis(R, k, Ecut, S):
+        gb = jd.jdft_basis_create(R, k, Ecut, S, device=local)
+        jd.jdft_alloc_workspace(gb, min(nb, args.ws_bands), max(nb, nproj))
+        return gb, jd.jdft_basis_export(gb)[0]
+
+    kdata, V, D = shard_inputs(args.config, layout, make_basis, lambda a: torch.from_numpy(a).cuda())
+    for d in kdata.values():
+        d["HC"] = torch.empty_like(d["C"])
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+
+    def step():
+        return sh.sharded_step(layout, kdata, V, D, group=group, mode=args.shard_mode, overlap=True)
+
+    def timed(n):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        for a, b in ev:
+            flush.zero_()
+            a.record()
+            step()
+            b.record()
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    timed(max(args.warmup, 3))
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    jd.jdft_launch_count(reset=True)
+    sampler = ClockSampler(local) if rank == 0 else None
+    times = timed(args.steps)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    ms_step = max_over_ranks(float(np.mean(times)), world)
+    if rank != 0:
+        return
+    line = {"metric": METRIC, "value": nb * nk / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "bands": nb, "kpoints": nk, "nproj": nproj,
+                       "parallelism": "kb-sharded x%d (k-points first, then bands; overlap by %s)" % (world, args.shard_mode),
+                       "units_of_rank0": layout.group_units(), "overlap_in_step": True,
+                       "l2": "flushed (512 MiB memset) before every timed step"},
+            "clocks": clocks, "gpu_launches": jd.jdft_launch_count(),
+            "roofline": None, "note": "sharded mode: per-kernel rooflines are reported by the default (replica) mode"}
+    print(json.dumps(line), flush=True)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -628,6 +716,9 @@ def main():
     ap.add_argument("--extras", action="store_true", help="also time the SURVEY 8(f) operations (density, subspace, Listing 1, ...)")
     ap.add_argument("--overlap", action="store_true",
                     help="run the projection GEMM on a side stream beside the FFT pipeline (measured +1-2 %%; off by default)")
+    ap.add_argument("--shard", default="", choices=["", "kb"],
+                    help="kb: ONE job sharded over the ranks by (k-point, band range) through sharding.py instead of N replicas")
+    ap.add_argument("--shard-mode", default="allgather", choices=["allgather", "ring"], help="schedule of the band-sharded overlap")
     ap.add_argument("--opt", action="append", default=[], help="library option key=value (jdft_set_option), repeatable; for experiments")
     ap.add_argument("--also", type=lambda s: [int(x) for x in s.split(",") if x], default=None,
                     help="other configs to attach as compact sub-records (default: 2,3,4 when --config is 5 and all defaults)")
@@ -639,7 +730,10 @@ def main():
         if int(os.environ.get("RANK", "0")) == 0:
             run_reference(args)
         return
-    run_ours(args)
+    if args.shard:
+        run_shard(args)
+    else:
+        run_ours(args)
     if int(os.environ.get("WORLD_SIZE", "1")) > 1:
         import torch.distributed as dist
         dist.destroy_process_group()

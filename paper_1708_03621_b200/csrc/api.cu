@@ -248,7 +248,12 @@ extern "C" int jdft_overlap_us(const jdft_basis *b, const double *P, int nproj, 
     // A1[a][j] = (P^+ C1)[j][a];  Bd[bb][j] = Omega (Q P^+ C2)[j][bb]
     if ((rc = jdft_gemm_dotk(b, C1, nb1, P, nproj, b->nG, 1, 1.0, nullptr, A1, part, part_bytes, st))) return rc;
     const double *Bd;
-    if ((rc = project_D(b, P, nproj, Q, Q_mode, C2, nb2, b->volume, B1, B2, part, part_bytes, st, &Bd))) return rc;
+    if (C1 == C2 && nb1 == nb2) {   // one projection serves both sides: Bd = Omega Q A1
+        if ((rc = jdft_apply_D(b, A1, nb1, nproj, Q, Q_mode, b->volume, B1, part, part_bytes, st))) return rc;
+        Bd = B1;
+    } else if ((rc = project_D(b, P, nproj, Q, Q_mode, C2, nb2, b->volume, B1, B2, part, part_bytes, st, &Bd))) {
+        return rc;
+    }
     // M[bb][a] += sum_j Bd[bb][j] conj(A1[a][j])
     return jdft_gemm_dotk(b, Bd, nb2, A1, nb1, nproj, 1, 1.0, nullptr, M, part, part_bytes, st, nullptr, 0, 1);
 }

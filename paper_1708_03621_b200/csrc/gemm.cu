@@ -520,6 +520,36 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     return JDFT_OK;
 }
 
+// Out[r][:] = scale * D . A[r][:] for projected coefficients A [Rn][Cn] that already exist (D_mode as in the ABI):
+// the reduction kernels with a single "partial" (diagonal / block-diagonal D) or one small GEMM (dense D)
+int jdft_apply_D(const jdft_basis *b, const double *A, int Rn, int Cn, const double *D, int D_mode, double scale, double *Out,
+                 void *scratch, size_t scratch_bytes, cudaStream_t st) {
+    if (Rn <= 0 || Cn <= 0) return JDFT_OK;
+    if (D_mode == 1) return jdft_gemm_dotk(b, A, Rn, D, Cn, Cn, 0, scale, nullptr, Out, scratch, scratch_bytes, st);
+    const int64_t total = (int64_t)Rn * Cn;
+    jdft_prof_begin(b, JDFT_K_REDUCE, st);
+    if (D_mode == 0) {
+        int64_t blocks = (total + 255) / 256;
+        if (blocks > b->num_sms * 8) blocks = b->num_sms * 8;
+        k_splitk_reduce<<<(int)blocks, 256, 0, st>>>((const double2 *)A, 1, total, Cn, scale, D, (double2 *)Out, 0, 0);
+    } else {
+        const int nblk = D_mode;
+        int64_t bl = ((int64_t)Rn * (Cn / nblk) + 127) / 128;
+        if (bl > b->num_sms * 8) bl = b->num_sms * 8;
+        if (nblk <= 4) k_splitk_reduce_block<4><<<(int)bl, 128, 0, st>>>((const double2 *)A, 1, Rn, Cn, nblk, scale, (const double2 *)D, (double2 *)Out);
+        else if (nblk <= 9) k_splitk_reduce_block<9><<<(int)bl, 128, 0, st>>>((const double2 *)A, 1, Rn, Cn, nblk, scale, (const double2 *)D, (double2 *)Out);
+        else if (nblk <= 16) k_splitk_reduce_block<16><<<(int)bl, 128, 0, st>>>((const double2 *)A, 1, Rn, Cn, nblk, scale, (const double2 *)D, (double2 *)Out);
+        else {
+            int64_t blocks = (total + 255) / 256;
+            if (blocks > b->num_sms * 8) blocks = b->num_sms * 8;
+            k_splitk_reduce_block_any<<<(int)blocks, 256, 0, st>>>((const double2 *)A, 1, Rn, Cn, nblk, scale, (const double2 *)D, (double2 *)Out);
+        }
+    }
+    jdft_prof_end(b, JDFT_K_REDUCE, st);
+    JDFT_LAUNCH_CHECK("apply_D");
+    return JDFT_OK;
+}
+
 int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
                      cudaStream_t st, const double *Add, double addscale) {
     if (Rn <= 0 || Nn <= 0) return JDFT_OK;

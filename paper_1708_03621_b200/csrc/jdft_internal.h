@@ -125,6 +125,8 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
                    double scale, const double *dscale, double *Out, void *scratch, size_t scratch_bytes,
                    cudaStream_t st, const double *dblock = nullptr, int nblk = 0, int accumulate = 0);
 // Out[r][n] (+)= sum_j A[r][j] * Pm[j][n];  A [Rn][K] (K contiguous), Pm [K][Nn] (n contiguous), Out [Rn][Nn]
+int jdft_apply_D(const jdft_basis *b, const double *A, int Rn, int Cn, const double *D, int D_mode, double scale, double *Out,
+                 void *scratch, size_t scratch_bytes, cudaStream_t st);
 // accumulate == 0 and Add != nullptr: Out = addscale * Add + A Pm  (Add [Rn][Nn]; may alias Out)
 int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double *Pm, int K, int64_t Nn, double *Out, int accumulate,
                      cudaStream_t st, const double *Add = nullptr, double addscale = 0.0);

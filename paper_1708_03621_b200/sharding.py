@@ -60,6 +60,14 @@ class KBLayout:
         self.group_size = len(self.group_ranks)
         self.group_rank = self.group_ranks.index(rank)
 
+    def group_units(self):
+        """Like `units`, but a member of a band group whose band range is empty still gets its (k, lo, lo) entry: it
+        has to take part in the group's collectives."""
+        if self.units or self.world <= self.nk:
+            return list(self.units)
+        blo, bhi = shard_range(self.nb, self.group_size, self.group_rank)
+        return [(self.group_index, blo, bhi)]
+
     def band_ranges(self):
         """Band range of every member of this rank's group, in group order."""
         return [shard_range(self.nb, self.group_size, i) for i in range(self.group_size)]
@@ -180,3 +188,22 @@ def sharded_density(basis, C_local, f_local, group=None, weight=1.0, n=None, ops
         return part
     n += part.view_as(n)
     return n
+
+
+def sharded_step(layout, kdata, Vloc, D, group=None, mode="allgather", overlap=True, ops=None):
+    """One pass of the hot path over this rank's (k-point, band range) units -- what `bench.py --shard kb` times.
+    `kdata[k] = dict(basis=..., P=..., C=<this rank's band rows of k-point k>, HC=<optional output>)`.
+    Per unit: `HC` for the local band columns (no collective) and, with `overlap`, this rank's column block
+    `M[:, lo:hi]` of `C^dagger O C` of that k-point (one all-gather or a ring over the band group).
+    Returns `{k: (HC_local, M_cols or None)}`."""
+    out = {}
+    for k, blo, bhi in layout.group_units():
+        d = kdata[k]
+        HC = d["C"].new_zeros(d["C"].shape) if bhi == blo else sharded_apply_H(d["basis"], Vloc, d["P"], D, d["C"], d.get("HC"), ops=ops)
+        M = None
+        if overlap and layout.group_size == 1:      # this rank holds all bands of the k-point: a local GEMM, no collective
+            M = (ops or _default_ops()).jdft_overlap(d["basis"], d["C"], d["C"])
+        elif overlap:
+            M = sharded_overlap(d["basis"], d["C"], d["C"], layout.nb, group=group, mode=mode, ops=ops)
+        out[k] = (HC, M)
+    return out

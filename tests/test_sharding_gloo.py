@@ -141,3 +141,80 @@ def test_kb_layout_k_first_then_bands():
                     assert (k, bnd) not in seen
                     seen.add((k, bnd))
         assert len(seen) == 40
+
+
+STEP_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %(root)r)
+import numpy as np, torch
+import torch.distributed as dist
+import bench, workloads
+from oracle import ref
+from paper_1708_03621_b200 import sharding as sh
+
+class OracleOps:   # stand-in for binding.jdft_* on CPU tensors (test infrastructure)
+    @staticmethod
+    def jdft_overlap(b, C1, C2):
+        return torch.from_numpy(np.ascontiguousarray(b.overlap(C1.numpy(), C2.numpy())))
+    @staticmethod
+    def jdft_apply_H(b, V, P, D, C, HC=None):
+        return torch.from_numpy(b.apply_H(V.numpy(), P.numpy(), D.numpy(), C.numpy()))
+
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+cfg_id = %(cfg)d
+cfg = workloads.get_config(cfg_id)
+nk, nb = len(cfg["kpoints"]), cfg["nb"]
+lay = sh.KBLayout(nk, nb, world, rank)
+grp = lay.new_band_group()
+def make_basis(R, k, Ecut, S):
+    b = ref.RefBasis(R, k, Ecut, S)
+    return b, b.iG
+kdata, V, D = bench.shard_inputs(cfg_id, lay, make_basis, torch.from_numpy)
+errs = {}
+for mode in ("allgather", "ring"):
+    out = sh.sharded_step(lay, kdata, V, D, group=grp, mode=mode, overlap=True, ops=OracleOps)
+    for k, blo, bhi in lay.group_units():
+        b = kdata[k]["basis"]
+        inp = workloads.make_inputs(cfg_id, b.iG, ik=k)
+        HC, M = out[k]
+        if bhi > blo:
+            want = b.apply_H(inp["Vloc"], inp["P"], inp["D"], inp["C"][blo:bhi])
+            errs["H_%%s_k%%d" %% (mode, k)] = float(np.abs(HC.numpy() - want).max() / np.abs(want).max())
+        wantM = b.overlap(inp["C"], inp["C"])[:, blo:bhi]
+        assert tuple(M.shape) == wantM.shape
+        errs["M_%%s_k%%d" %% (mode, k)] = float(np.abs(M.numpy() - wantM).max()) if wantM.size else 0.0
+dist.barrier()
+print(json.dumps({"rank": rank, "units": lay.group_units(), "errs": errs}), flush=True)
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("world,cfg", [(2, 103), (3, 103), (2, 101)])
+def test_bench_shard_mode_step_gloo(tmp_path, ref, world, cfg):
+    """The step `bench.py --shard kb` times (bench.shard_inputs + sharding.sharded_step), on gloo ranks with the oracle as
+    the local operation: shape 103 has 2 k-points (2 ranks: one k-point each, no collective; 3 ranks: k-point 0 on one
+    rank, k-point 1 band-sharded over two), shape 101 has one k-point and 5 bands over 2 ranks (ragged)."""
+    import json
+    script = tmp_path / "step_worker.py"
+    script.write_text(STEP_WORKER % {"root": ROOT, "cfg": cfg})
+    port = _free_port()
+    procs = []
+    for r in range(world):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), OMP_NUM_THREADS="1")
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True))
+    units = []
+    for p in procs:
+        out, err = p.communicate(timeout=400)
+        assert p.returncode == 0, err[-3000:]
+        o = json.loads(out.strip().splitlines()[-1])
+        units += [tuple(u) for u in o["units"]]
+        assert o["errs"], "rank did no work"
+        for name, e in o["errs"].items():
+            assert e <= 1e-12, (name, e)
+    # every (k, band) of the job is covered exactly once
+    cfgd = __import__("workloads").get_config(cfg)
+    covered = sorted((k, bnd) for k, lo, hi in units for bnd in range(lo, hi))
+    assert covered == [(k, bnd) for k in range(len(cfgd["kpoints"])) for bnd in range(cfgd["nb"])]

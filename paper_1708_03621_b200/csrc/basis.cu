@@ -9,6 +9,7 @@
 #include <new>
 #include <utility>
 #include "jdft_internal.h"
+#include "tma.cuh"
 
 static thread_local char g_err[512] = "";
 static thread_local int64_t g_launches = 0;
@@ -48,6 +49,19 @@ cudaError_t jdft_ensure_smem(const void *kernel, size_t bytes, int device) {
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     if (e == cudaSuccess) have = bytes;
     return e;
+}
+
+JdftEncodeTiledFn jdft_tensor_map_encoder() {
+    static JdftEncodeTiledFn fn = []() -> JdftEncodeTiledFn {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        return (JdftEncodeTiledFn)p;
+    }();
+    return fn;
 }
 
 static bool smooth235(int n) {
@@ -151,7 +165,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     b->h_ops_set = 0; b->h_nproj = 0; b->h_D_mode = 0;
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
     b->opt_profile_kernel = 0; b->prof_used = 0;
-    b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_gemm3m = 1; b->opt_tma = 0; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
+    b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_gemm3m = 1; b->opt_tma = 0; b->opt_gemm_tma = 0; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
 
     // G = 2 pi R^-1 (adjugate / det): row i of G is the reciprocal vector b_i
     {
@@ -369,8 +383,9 @@ extern "C" int jdft_set_option(jdft_basis *b, const char *key, int64_t value) {
     if (!strcmp(key, "band_batch")) { b->opt_band_batch = value < 0 ? 0 : value; return JDFT_OK; }
     if (!strcmp(key, "planes_pair")) { b->opt_pair = value != 0; return JDFT_OK; }
     if (!strcmp(key, "planes_prune")) { b->opt_prune = value != 0; return JDFT_OK; }
+    if (!strcmp(key, "gemm_tma")) { b->opt_gemm_tma = value != 0; return JDFT_OK; }
     if (!strcmp(key, "planes_tma")) { b->opt_tma = value != 0; return JDFT_OK; }
-    if (!strcmp(key, "gemm_3m")) { b->opt_gemm3m = value != 0; return JDFT_OK; }
+    if (!strcmp(key, "gemm_3m")) { b->opt_gemm3m = value < 0 ? 0 : value; return JDFT_OK; }
     if (!strcmp(key, "overlap_gemm")) { b->opt_overlap = value != 0; return JDFT_OK; }
     if (!strcmp(key, "force_generic_fft")) { b->opt_force_generic = value != 0; return JDFT_OK; }
     if (!strcmp(key, "profile_kernel")) { b->opt_profile_kernel = value; b->prof_used = 0; return JDFT_OK; }

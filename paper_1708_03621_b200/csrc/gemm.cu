@@ -9,7 +9,9 @@
 // Tiles: 64 x 64 per CTA, 4 warps of 32 x 32 (4 x 4 DMMA tiles of 8 x 8), BK = 8, 4-stage cp.async pipeline.
 // Shared-memory layout of a K-contiguous operand: per group of 4 k, a dense [64 rows][4 k] block of c128
 // (64 B per row, so the 8 lanes of a quarter-warp read 128 contiguous bytes), blocks skewed by 64 B.
+#include <cstring>
 #include "jdft_internal.h"
+#include "tma.cuh"
 
 namespace {
 
@@ -35,11 +37,12 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, const double a, con
 }
 
 // load one stage of a K-contiguous operand: rows [row0, row0+64) of M [nrows][ld], k in [k0, k0+BK), zero beyond kend/nrows
-template <int BKT = BK>
+template <int BKT = BK, int ROWS = 64>   // ROWS: rows of the tile that are used (the rest of the 64-row block is never read)
 __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld, int nrows, int row0, int64_t k0,
                                          int64_t kend, int tid) {
+    static_assert((ROWS * BKT) % NTHREADS == 0, "whole rounds");
 #pragma unroll
-    for (int i = 0; i < (64 * BKT) / NTHREADS; i++) {
+    for (int i = 0; i < (ROWS * BKT) / NTHREADS; i++) {
         const int e = tid + i * NTHREADS;
         const int r = e / BKT, kk = e % BKT;
         const int64_t k = k0 + kk;
@@ -51,18 +54,25 @@ __device__ __forceinline__ void load_opk(char *dst, const double2 *M, int64_t ld
 
 // ---------------------------------------------------------------------------------------------- dot-K GEMM
 // BN_ = 64, or 48 when the column extent is a multiple of 48 but not of 64 (np = 288, 864: no zero-padded DMMAs)
-// M3: the complex product by the 3M (Gauss) scheme -- three real DMMAs per complex tile product instead of four:
-//   k1 = (xr + xi) yr,  k2 = xr (e - yr),  k3 = xi (yr + e)   (e = +-yi),   real = k1 - k3,  imag = k1 + k2
-// (three accumulator sets; the two operand sums cost 1 + 2/MT DADD per fragment).  Normwise as accurate as the 4M
+// M3: the complex product by the 3M (Karatsuba) scheme -- three real DMMAs per complex tile product instead of four:
+//   t1 = xr yr,  t2 = xi e,  t3 = (xr + xi)(yr + e)   (e = +-yi),   real = t1 - t2,  imag = t3 - t1 - t2
+// (three accumulator sets; one operand sum per fragment).  Normwise as accurate as the 4M
 // scheme (Higham, Accuracy and Stability, ch. 23: 3M is normwise stable), which is what the per-band relative L2
 // tolerance measures; 25 % fewer tensor instructions.
-template <bool CONJY, bool TRI, int BN_, bool M3 = false, int ST = STAGES, int BKT = BK>
-__global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double2 *__restrict__ X, const int Rn,
+// TMA: the operand stages are filled by cp.async.bulk.tensor (one elected thread, 2 D boxes {4 k, rows} that land as the
+// same [rows][4] blocks the fragment loads expect, mbarrier-signalled, out-of-range rows / k zero-filled by the TMA unit)
+// instead of 7 predicated cp.async with 64-bit address arithmetic per thread and k-tile.
+template <bool CONJY, bool TRI, int BN_, bool M3 = false, int ST = STAGES, int BKT = BK, bool TMA = false>
+__global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const __grid_constant__ CUtensorMap tmX,
+                                                        const __grid_constant__ CUtensorMap tmY,
+                                                        const double2 *__restrict__ X, const int Rn,
                                                         const double2 *__restrict__ Y, const int Cn, const int64_t K,
                                                         const int ktiles_per_split, double2 *__restrict__ part) {
-    extern __shared__ __align__(16) char smem[];
-    constexpr int OPKT = (BKT / 4) * KBLK_BYTES;   // one stage of a K-contiguous operand
+    extern __shared__ __align__(128) char smem[];
+    constexpr int KBLK = TMA ? 64 * 64 : KBLK_BYTES;   // pitch of one [64][4] block (the skew only serves cp.async writes)
+    constexpr int OPKT = (BKT / 4) * KBLK;             // one stage of a K-contiguous operand
     char *sX = smem, *sY = smem + ST * OPKT;
+    __shared__ __align__(8) uint64_t full[ST];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NTL = BN_ / 16;   // 8-wide DMMA tiles per warp along the columns
     const int wr = (warp >> 1) * 32, wc = (warp & 1) * (BN_ / 2);
@@ -100,23 +110,49 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
             if constexpr (M3) c3[i][j][0] = c3[i][j][1] = 0.0;
         }
 
-    for (int s = 0; s < ST - 1; s++) {
-        if (s < nkt) {
-            load_opk<BKT>(sX + s * OPKT, X, K, Rn, row0, (kt0 + s) * BKT, K, tid);
-            load_opk<BKT>(sY + s * OPKT, Y, K, cend, col0, (kt0 + s) * BKT, K, tid);
+    // one stage: (BKT / 4) boxes of {4 k, 64 rows} for X and {4 k, BN_ rows} for Y
+    auto tma_stage = [&](int slot, int64_t kt) {
+        constexpr uint32_t bytes = (BKT / 4) * (64 + BN_) * 64;
+        jtma::mbar_expect_tx(&full[slot], bytes);
+#pragma unroll
+        for (int q = 0; q < BKT / 4; q++) {
+            const int c0 = (int)(2 * (kt * BKT + 4 * q));   // coordinate in doubles along K
+            jtma::tma_load_2d(sX + slot * OPKT + q * KBLK, &tmX, c0, row0, &full[slot]);
+            jtma::tma_load_2d(sY + slot * OPKT + q * KBLK, &tmY, c0, col0, &full[slot]);
         }
-        cp_async_commit();
+    };
+    if constexpr (TMA) {
+        if (tid == 0) {
+            for (int s = 0; s < ST; s++) jtma::mbar_init(&full[s], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+        if (tid == 0)
+            for (int s = 0; s < ST - 1 && s < nkt; s++) tma_stage(s, kt0 + s);
+    } else {
+        for (int s = 0; s < ST - 1; s++) {
+            if (s < nkt) {
+                load_opk<BKT>(sX + s * OPKT, X, K, Rn, row0, (kt0 + s) * BKT, K, tid);
+                load_opk<BKT, BN_>(sY + s * OPKT, Y, K, cend, col0, (kt0 + s) * BKT, K, tid);
+            }
+            cp_async_commit();
+        }
     }
     const int fo = (lane >> 2) * 64 + (lane & 3) * 16;  // fragment offset inside a [64][4] block
     for (int kt = 0; kt < nkt; kt++) {
-        cp_async_wait<ST - 2>();
-        __syncthreads();
-        {
+        if constexpr (TMA) {
+            jtma::mbar_wait(&full[kt % ST], (kt / ST) & 1);
+            __syncthreads();   // everyone is done with the stage of k-tile kt - 1, which is refilled now
+            const int nx = kt + ST - 1;
+            if (tid == 0 && nx < nkt) tma_stage(nx % ST, kt0 + nx);
+        } else {
+            cp_async_wait<ST - 2>();
+            __syncthreads();
             const int nx = kt + ST - 1;
             if (nx < nkt) {
                 const int slot = nx % ST;
                 load_opk<BKT>(sX + slot * OPKT, X, K, Rn, row0, (kt0 + nx) * BKT, K, tid);
-                load_opk<BKT>(sY + slot * OPKT, Y, K, cend, col0, (kt0 + nx) * BKT, K, tid);
+                load_opk<BKT, BN_>(sY + slot * OPKT, Y, K, cend, col0, (kt0 + nx) * BKT, K, tid);
             }
             cp_async_commit();
         }
@@ -126,27 +162,26 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
             double2 a[4], bq[NTL];
 #pragma unroll
             for (int i = 0; i < 4; i++)
-                a[i] = *reinterpret_cast<const double2 *>(bx + kk * KBLK_BYTES + (wr + 8 * i) * 64 + fo);
+                a[i] = *reinterpret_cast<const double2 *>(bx + kk * KBLK + (wr + 8 * i) * 64 + fo);
 #pragma unroll
             for (int j = 0; j < NTL; j++)
-                bq[j] = *reinterpret_cast<const double2 *>(by + kk * KBLK_BYTES + (wc + 8 * j) * 64 + fo);
+                bq[j] = *reinterpret_cast<const double2 *>(by + kk * KBLK + (wc + 8 * j) * 64 + fo);
             if constexpr (M3) {
-                double sa[4], d2[NTL], s3[NTL];
+                double sa[4], sb[NTL], e[NTL];
 #pragma unroll
                 for (int i = 0; i < 4; i++) sa[i] = a[i].x + a[i].y;
 #pragma unroll
                 for (int j = 0; j < NTL; j++) {
-                    const double e = CONJY ? -bq[j].y : bq[j].y;   // X (yr + i e)
-                    d2[j] = e - bq[j].x;
-                    s3[j] = bq[j].x + e;
+                    e[j] = CONJY ? -bq[j].y : bq[j].y;   // X (yr + i e)
+                    sb[j] = bq[j].x + e[j];
                 }
 #pragma unroll
                 for (int i = 0; i < 4; i++)
 #pragma unroll
                     for (int j = 0; j < NTL; j++) {
-                        dmma(cr[i][j][0], cr[i][j][1], sa[i], bq[j].x);
-                        dmma(ci[i][j][0], ci[i][j][1], a[i].x, d2[j]);
-                        dmma(c3[i][j][0], c3[i][j][1], a[i].y, s3[j]);
+                        dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);   // t1 = xr yr
+                        dmma(ci[i][j][0], ci[i][j][1], a[i].y, e[j]);      // t2 = xi e
+                        dmma(c3[i][j][0], c3[i][j][1], sa[i], sb[j]);      // t3 = (xr + xi)(yr + e)
                     }
             } else {
 #pragma unroll
@@ -170,12 +205,12 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const double
             for (int j = 0; j < NTL; j++)
 #pragma unroll
                 for (int h = 0; h < 2; h++) {
-                    const double k1 = cr[i][j][h], k2 = ci[i][j][h], k3 = c3[i][j][h];
-                    cr[i][j][h] = k1 - k3;
-                    ci[i][j][h] = k1 + k2;
+                    const double t1 = cr[i][j][h], t2 = ci[i][j][h], t3 = c3[i][j][h];
+                    cr[i][j][h] = t1 - t2;
+                    ci[i][j][h] = (t3 - t1) - t2;
                 }
     }
-    cp_async_wait<0>();
+    if constexpr (!TMA) cp_async_wait<0>();
     double2 *P = part + (size_t)blockIdx.z * Rn * Cn;
 #pragma unroll
     for (int i = 0; i < 4; i++) {
@@ -294,9 +329,18 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
     char *sA = smem, *sP = smem + ST * OPK_BYTES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wr = (warp / WN) * (8 * MTL), wc = (warp % WN) * (8 * NTL);
-    const int row0 = blockIdx.y * BM;
-    const int64_t n0 = (int64_t)blockIdx.x * BN_;
+    // row tile fastest: the CTAs that share one n-tile of P (all band tiles) run at the same time, so P comes from HBM
+    // once and from L2 otherwise (ncu, config 5: 14.7 GB of DRAM reads per launch with the n-tile fastest)
+    const int row0 = blockIdx.x * BM;
+    const int64_t n0 = (int64_t)blockIdx.y * BN_;
     const int nkt = (K + BK - 1) / BK;
+    if (Add) {   // pull the tile the epilogue adds to towards L2 while the main loop runs
+        for (int e = tid; e < BM * ((BN_ * 16 + 127) / 128); e += NTHREADS) {
+            const int r = e / ((BN_ * 16 + 127) / 128), seg = e % ((BN_ * 16 + 127) / 128);
+            if (row0 + r < Rn && n0 + seg * 8 < Nn)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(Add + (size_t)(row0 + r) * Nn + n0 + seg * 8));
+        }
+    }
 
     double cr[MTL][NTL][2], ci[MTL][NTL][2], c3[M3 ? MTL : 1][M3 ? NTL : 1][2];   // 3M: k1, k2, k3 (see k_gemm_dotk)
 #pragma unroll
@@ -350,21 +394,18 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
             for (int j = 0; j < NTL; j++)
                 bq[j] = *reinterpret_cast<const double2 *>(bp + kk * 4 * PROW + (wc + 8 * j) * 16 + fp);
             if constexpr (M3) {
-                double sa[MTL], d2[NTL], s3[NTL];
+                double sa[MTL], sb[NTL];
 #pragma unroll
                 for (int i = 0; i < MTL; i++) sa[i] = a[i].x + a[i].y;
 #pragma unroll
-                for (int j = 0; j < NTL; j++) {
-                    d2[j] = bq[j].y - bq[j].x;
-                    s3[j] = bq[j].x + bq[j].y;
-                }
+                for (int j = 0; j < NTL; j++) sb[j] = bq[j].x + bq[j].y;
 #pragma unroll
                 for (int i = 0; i < MTL; i++)
 #pragma unroll
                     for (int j = 0; j < NTL; j++) {
-                        dmma(cr[i][j][0], cr[i][j][1], sa[i], bq[j].x);
-                        dmma(ci[i][j][0], ci[i][j][1], a[i].x, d2[j]);
-                        dmma(c3[i][j][0], c3[i][j][1], a[i].y, s3[j]);
+                        dmma(cr[i][j][0], cr[i][j][1], a[i].x, bq[j].x);
+                        dmma(ci[i][j][0], ci[i][j][1], a[i].y, bq[j].y);
+                        dmma(c3[i][j][0], c3[i][j][1], sa[i], sb[j]);
                     }
             } else {
 #pragma unroll
@@ -387,9 +428,9 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
             for (int j = 0; j < NTL; j++)
 #pragma unroll
                 for (int h = 0; h < 2; h++) {
-                    const double k1 = cr[i][j][h], k2 = ci[i][j][h], k3 = c3[i][j][h];
-                    cr[i][j][h] = k1 - k3;
-                    ci[i][j][h] = k1 + k2;
+                    const double t1 = cr[i][j][h], t2 = ci[i][j][h], t3 = c3[i][j][h];
+                    cr[i][j][h] = t1 - t2;
+                    ci[i][j][h] = (t3 - t1) - t2;
                 }
     }
 #pragma unroll
@@ -437,7 +478,7 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     // 3M scheme (three DMMAs per complex tile product; 64 x 48 tiles, its three accumulator sets leave no room for
     // 64 x 64): taken when 0.8 x its padded width beats the 4M choice and K is long enough to matter
     const bool m3 = b->opt_gemm3m && K >= 512 && (tri ? Cn >= 128 : pad48 * 80 < (bn == 48 ? pad48 : pad64) * 100);
-    if (m3) bn = 48;
+    if (m3) bn = 48;   // (64 x 32 tiles at 3 CTAs per SM measured 7 % slower)
     // pipeline of the 3M kernels: measured on config 3 (P^+ C, 1.70 ms): 6 stages of 8 -> 1.78 ms, 3 stages of 16 -> 1.89 ms
     constexpr int ST3 = STAGES, BK3 = BK;
     const int bk = m3 ? BK3 : BK;
@@ -476,16 +517,36 @@ int jdft_gemm_dotk(const jdft_basis *b, const double *X, int Rn, const double *Y
     if (per < 1) per = 1;
     nsplit = (ktiles + per - 1) / per;
     if (nsplit < 1) nsplit = 1;
-    const size_t smem = m3 ? 2 * ST3 * (BK3 / 4) * KBLK_BYTES : 2 * STAGES * OPK_BYTES;
+    // TMA operand staging (option "gemm_tma"): both operands need 16-byte aligned rows (K even or ... always: c128) and
+    // extents that fit the tensor-map fields; the 3M kernels only (they are the ones on the hot path)
+    CUtensorMap tmX, tmY;
+    memset(&tmX, 0, sizeof(tmX));
+    memset(&tmY, 0, sizeof(tmY));
+    bool tma = false;
+    if (m3 && b->opt_gemm_tma && K < ((int64_t)1 << 30)) {
+        JdftEncodeTiledFn enc = jdft_tensor_map_encoder();
+        const cuuint64_t strX[1] = {(cuuint64_t)K * 16};
+        const cuuint64_t dimX[2] = {(cuuint64_t)2 * K, (cuuint64_t)Rn}, dimY[2] = {(cuuint64_t)2 * K, (cuuint64_t)Cn};
+        const cuuint32_t boxX[2] = {8, 64}, boxY[2] = {8, (cuuint32_t)bn}, es[2] = {1, 1};
+        tma = enc &&
+              enc(&tmX, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void *)X, dimX, strX, boxX, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS &&
+              enc(&tmY, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void *)Y, dimY, strX, boxY, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    }
+    const size_t smem = m3 ? 2 * ST3 * (BK3 / 4) * (tma ? 4096 : KBLK_BYTES) + (tma ? 128 : 0) : 2 * STAGES * OPK_BYTES;
     dim3 grid(tri ? tiles : tcol, tri ? 1 : trow, (unsigned)nsplit);
     jdft_prof_begin(b, JDFT_K_GEMM_DOTK, st);
 #define JDFT_DOTK_LAUNCH(...)                                                                                  \
     do {                                                                                                        \
         JDFT_CUDA(ensure_smem(k_gemm_dotk<__VA_ARGS__>, smem, b->device));                                      \
-        k_gemm_dotk<__VA_ARGS__><<<grid, NTHREADS, smem, st>>>((const double2 *)X, Rn, (const double2 *)Y, Cn, K, \
+        k_gemm_dotk<__VA_ARGS__><<<grid, NTHREADS, smem, st>>>(tmX, tmY, (const double2 *)X, Rn, (const double2 *)Y, Cn, K, \
                                                                (int)per, (double2 *)scratch);                  \
     } while (0)
-    if (tri && m3) JDFT_DOTK_LAUNCH(true, true, 48, true, ST3, BK3);
+    if (tri && m3 && tma) JDFT_DOTK_LAUNCH(true, true, 48, true, ST3, BK3, true);
+    else if (m3 && tma && conjY) JDFT_DOTK_LAUNCH(true, false, 48, true, ST3, BK3, true);
+    else if (m3 && tma) JDFT_DOTK_LAUNCH(false, false, 48, true, ST3, BK3, true);
+    else if (tri && m3) JDFT_DOTK_LAUNCH(true, true, 48, true, ST3, BK3);
     else if (tri) JDFT_DOTK_LAUNCH(true, true, 64);
     else if (m3 && conjY) JDFT_DOTK_LAUNCH(true, false, 48, true, ST3, BK3);
     else if (m3) JDFT_DOTK_LAUNCH(false, false, 48, true, ST3, BK3);
@@ -566,18 +627,18 @@ int jdft_gemm_expand(const jdft_basis *b, const double *A, int Rn, const double 
         constexpr int BNX = 48, ST3 = 6;
         const size_t smem = ST3 * (OPK_BYTES + BK * (BNX * 16 + 32));
         JDFT_CUDA(ensure_smem(k_gemm_expand<BNX, 2, 2, true, ST3>, smem, b->device));
-        dim3 grid((unsigned)((Nn + BNX - 1) / BNX), (unsigned)rt);
+        dim3 grid((unsigned)rt, (unsigned)((Nn + BNX - 1) / BNX));
         k_gemm_expand<BNX, 2, 2, true, ST3><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, (const double2 *)Add, addscale);
     } else if (narrow) {
         constexpr int BNX = 56;
         const size_t smem = STAGES * (OPK_BYTES + BK * (BNX * 16 + 32));
         JDFT_CUDA(ensure_smem(k_gemm_expand<BNX, 4, 1>, smem, b->device));
-        dim3 grid((unsigned)((Nn + BNX - 1) / BNX), (unsigned)rt);
+        dim3 grid((unsigned)rt, (unsigned)((Nn + BNX - 1) / BNX));
         k_gemm_expand<BNX, 4, 1><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, (const double2 *)Add, addscale);
     } else {
         const size_t smem = STAGES * (OPK_BYTES + OPN_BYTES);
         JDFT_CUDA(ensure_smem(k_gemm_expand<BN, 2, 2>, smem, b->device));
-        dim3 grid((unsigned)((Nn + BN - 1) / BN), (unsigned)rt);
+        dim3 grid((unsigned)rt, (unsigned)((Nn + BN - 1) / BN));
         k_gemm_expand<BN, 2, 2><<<grid, NTHREADS, smem, st>>>((const double2 *)A, Rn, (const double2 *)Pm, K, Nn, (double2 *)Out, (const double2 *)Add, addscale);
     }
     jdft_prof_end(b, JDFT_K_GEMM_EXPAND, st);

@@ -7,7 +7,7 @@
 //   K5 k_cols_fwd   forward FFT along axis 2 (+) gather box -> sphere (+) + Omega ke C   (the -1/2 L C term)
 // Intermediates: W1 [nbatch][ncol][S2] and W2 [nbatch][npl][S1][S2] (c128) in the caller's workspace.
 #include <cmath>
-#include <cuda.h>
+#include "tma.cuh"
 #include "fft.cuh"
 #include "cols_tuned.cuh"
 
@@ -1220,23 +1220,6 @@ bool planes_prunable(const jdft_basis *b, int L) {
     return C::R1 == 8 && b->opt_prune && b->m0lo < 0 && b->m0lo + b->npl <= 2 * C::R2 && L + b->m0lo >= 6 * C::R2;
 }
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
-                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-EncodeTiledFn tensor_map_encoder() {
-    static EncodeTiledFn fn = []() -> EncodeTiledFn {
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
-            cudaGetLastError();
-            return nullptr;
-        }
-        return (EncodeTiledFn)p;
-    }();
-    return fn;
-}
-
 // K3 through TMA (planes_tma.cuh): returns 1 if launched, 0 if this shape / pointer cannot take the path, < 0 on error
 template <int LT>
 int try_planes_tma(const jdft_basis *b, int nbt, double2 *W2, const double *V, cudaStream_t st) {
@@ -1245,7 +1228,7 @@ int try_planes_tma(const jdft_basis *b, int nbt, double2 *W2, const double *V, c
     } else {
         using Q = PlanesTma<LT>;
         const int S1 = b->S[1], S2 = b->S[2], npl = b->npl;
-        EncodeTiledFn enc = tensor_map_encoder();
+        JdftEncodeTiledFn enc = jdft_tensor_map_encoder();
         const size_t smem = Q::smem_bytes(npl);
         if (!enc || !b->opt_tma || npl > 256 || S1 > 65536 || smem > 200 * 1024 || (((uintptr_t)W2) & 15)) return 0;
         CUtensorMap tm;

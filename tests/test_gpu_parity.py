@@ -623,8 +623,9 @@ def test_gemm_3m_and_4m_schemes_match_the_oracle(ref, jd, cfg_id):
     C2 = np.ascontiguousarray(c.C[::-1] * (1.0 + 0.5j)) + 0.1 * rng.standard_normal(c.C.shape)
     wantM = c.rb.overlap(c.C, C2)
     res = {}
-    for m3 in (0, 1):
-        jd.jdft_set_option(c.gb, "gemm_3m", m3)
+    for m3 in (0, 1, 2):                                      # 2: the 3M kernels with TMA operand staging ("gemm_tma")
+        jd.jdft_set_option(c.gb, "gemm_3m", min(m3, 1))
+        jd.jdft_set_option(c.gb, "gemm_tma", 1 if m3 == 2 else 0)
         got = jd.jdft_apply_Vnl(c.gb, dev(c.P), dev(c.D), dev(c.C)).cpu().numpy()
         assert rel_err_per_band(got, want) <= TOL
         B = jd.jdft_project(c.gb, dev(c.P), dev(c.C)).cpu().numpy()
@@ -633,6 +634,14 @@ def test_gemm_3m_and_4m_schemes_match_the_oracle(ref, jd, cfg_id):
         assert rel_err_per_band(M.T, wantM.T) <= TOL
         res[m3] = got
     assert rel_err_per_band(res[0], res[1]) <= 1e-12
+    assert rel_err_per_band(res[2], res[1]) <= 1e-13
+    # the Hermitian-triangle overlap through the TMA-staged kernel
+    Cn = workloads.make_bands(cfg_id, c.rb.nG, nb=130, orthonormalise=False)
+    jd.jdft_alloc_workspace(c.gb, 1, 130)
+    jd.jdft_set_option(c.gb, "gemm_tma", 1)
+    dCn = dev(Cn)
+    M = jd.jdft_overlap(c.gb, dCn, dCn).cpu().numpy()
+    assert rel_err_per_band(M.T, c.rb.overlap(Cn, Cn).T) <= TOL
 
 
 # ------------------------------------------------------------------------------------------ K3 through TMA

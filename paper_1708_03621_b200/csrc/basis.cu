@@ -398,7 +398,7 @@ int jdft_band_batch(const jdft_basis *b, int nb, size_t ws_offset) {
     size_t fit = (b->ws_bytes - ws_offset) / per;
     int64_t want = b->opt_band_batch;
     if (want <= 0) {
-        // automatic: as many bands as the workspace holds, up to 256.  Measured on B200 (profiles/r01_batch_sweep.md):
+        // automatic: as many bands as the workspace holds, up to 256.  Measured on B200 (band-batch sweep):
         // filling the GPU (thousands of CTAs per launch, few tail waves) beats keeping a small batch L2-resident.
         want = 256;
     }

@@ -235,7 +235,7 @@ __device__ __forceinline__ void twiddle_rows(double2 (&a)[R], const double2 *__r
     }
 }
 
-// resident CTAs per SM the register allocation of k_planes_fused is bounded for (measured: profiles/r01_planes_tuning.md)
+// resident CTAs per SM the register allocation of k_planes_fused is bounded for (measured: DESIGN.md section 12, table of experiments)
 // default: registers the fused middle radix needs (16 complex values + V factors for radix 15/16) against 64 K per SM
 template <int LT> struct PlanesMinB {
     static constexpr int need = Tuned<LT>::R2 >= 12 ? 128 : 96;

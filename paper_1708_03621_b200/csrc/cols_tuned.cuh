@@ -126,12 +126,27 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tun
     const int nbeg = s_n0[0], nend = s_n0[nc];
     {
         // scatter the sphere runs of the nc columns (contiguous in n) into the tile; nothing else of it is read
-        for (int e = tid; e < nend - nbeg; e += NT) {
-            const int n = nbeg + e;
-            const int t = find_col<T>(s_n0, n);
-            int row = s_m2w[t] + (n - s_n0[t]);
-            if (row >= L) row -= L;
-            X[F::sw(row, t)] = Cb[n];
+        // (the sphere reads are issued four deep before the first dependent shared-memory store: their HBM latency was
+        //  the largest single stall of the kernel in the ncu source page)
+        constexpr int U = F::NP == 3 ? 1 : 4;   // measured: pays at 128 (0.874 -> 0.847 ms) and 80, not at 216 (40 registers)
+        for (int e0 = tid; e0 < nend - nbeg; e0 += U * NT) {
+            double2 v[U];
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const int e = e0 + u * NT;
+                if (e < nend - nbeg) v[u] = Cb[nbeg + e];
+            }
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const int e = e0 + u * NT;
+                if (e < nend - nbeg) {
+                    const int n = nbeg + e;
+                    const int t = find_col<T>(s_n0, n);
+                    int row = s_m2w[t] + (n - s_n0[t]);
+                    if (row >= L) row -= L;
+                    X[F::sw(row, t)] = v[u];
+                }
+            }
         }
         __syncthreads();
         // pass 0 (radix R0, s = 1), in place: rows bf + k NB0 (zero outside the run) -> rows bf R0 + j; every round is
@@ -201,6 +216,19 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_FWD) k_cols_fwd_tun
     const int nc = min(T, ncol - c0);
     if (tid <= T) s_n0[tid] = col_n0[min(c0 + tid, ncol)];
     if (tid < T) s_m2w[tid] = wrap_row(col_m2lo[min(c0 + tid, ncol - 1)], L);
+    if (kin != 0.0 && LT == 128) {   // measured: 1.126 -> 1.116 ms at 128; slower at 80 and 216
+        // the gather at the end reads C and ke of this CTA's sphere run (contiguous in n) straight from HBM, and nothing
+        // hides that latency there (ncu: 45 % of the warp samples on long-scoreboard stalls): ask L2 for those lines now,
+        // one prefetch per thread, so they arrive while the transform runs
+        const int pb = __ldg(col_n0 + c0), pe = __ldg(col_n0 + min(c0 + T, ncol));
+        const char *pc = reinterpret_cast<const char *>(C + (size_t)b * nG + pb);
+        const char *pk = reinterpret_cast<const char *>(ke + pb);
+        const int nc_lines = ((pe - pb) * 16 + 127) / 128, nk_lines = ((pe - pb) * 8 + 127) / 128;
+        for (int e = tid; e < nc_lines + nk_lines; e += NT) {
+            const char *a = e < nc_lines ? pc + e * 128 : pk + (e - nc_lines) * 128;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+        }
+    }
     // pass 0 (radix R0, s = 1): lanes run along the pencil, inputs straight from W1[column][row]
     const double2 *Wb = W1 + ((size_t)b * ncol + c0) * L;
     {
@@ -232,21 +260,34 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_FWD) k_cols_fwd_tun
     const int nbeg = s_n0[0], nend = s_n0[nc];
     const double2 *Cb = C + (size_t)b * nG;
     double2 *Ob = outC + (size_t)b * nG;
-    for (int e = tid; e < nend - nbeg; e += NT) {
-        const int n = nbeg + e;
-        const int t = find_col<T>(s_n0, n);
-        int row = s_m2w[t] + (n - s_n0[t]);
-        if (row >= L) row -= L;
-        double2 v = X[F::sw(row, t)];
-        v.x *= scale;
-        v.y *= scale;
-        if (kin != 0.0) {
-            const double f = kin * ke[n];
-            const double2 c = Cb[n];
-            v.x = fma(f, c.x, v.x);
-            v.y = fma(f, c.y, v.y);
+    constexpr int U = LT == 128 ? 4 : 1;   // global reads of C and ke U deep, then the shared-memory gathers and the stores
+    for (int e0 = tid; e0 < nend - nbeg; e0 += U * NT) {
+        double2 c[U];
+        double f[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int e = e0 + u * NT;
+            c[u] = make_double2(0.0, 0.0);
+            f[u] = 0.0;
+            if (kin != 0.0 && e < nend - nbeg) {
+                c[u] = Cb[nbeg + e];
+                f[u] = kin * ke[nbeg + e];
+            }
         }
-        Ob[n] = v;
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int e = e0 + u * NT;
+            if (e < nend - nbeg) {
+                const int n = nbeg + e;
+                const int t = find_col<T>(s_n0, n);
+                int row = s_m2w[t] + (n - s_n0[t]);
+                if (row >= L) row -= L;
+                double2 v = X[F::sw(row, t)];
+                v.x = fma(f[u], c[u].x, v.x * scale);
+                v.y = fma(f[u], c[u].y, v.y * scale);
+                Ob[n] = v;
+            }
+        }
     }
 }
 

@@ -406,7 +406,7 @@ def measure(cfg_id, args, rank, world, local, full):
             for k, h in zip(ks, host):
                 jd.jdft_apply_H_host_resident(k["gb"], h["C"], h["HC"])
                 if do_overlap:
-                    jd.jdft_overlap_host(k["gb"], h["C"], h["C"], h["M"])
+                    jd.jdft_overlap_host_resident(k["gb"], h["M"])
 
         step_host_res()
         torch.cuda.synchronize()
@@ -417,8 +417,8 @@ def measure(cfg_id, args, rank, world, local, full):
         res_ms = max_over_ranks(1e3 * (time.perf_counter() - t0) / e2e_steps, world)
         e2e["resident_operators"] = {
             "value": aggregate_value(units, world, res_ms), "ms_per_step": res_ms,
-            "h2d_bytes_per_step": sum(h["C"].numel() * 16 * (2 if do_overlap else 1) for h in host), "d2h_bytes_per_step": d2h,
-            "note": "jdft_host_set_operators once, then jdft_apply_H_host_resident (+ jdft_overlap_host) per step"}
+            "h2d_bytes_per_step": sum(h["C"].numel() * 16 for h in host), "d2h_bytes_per_step": d2h,
+            "note": "jdft_host_set_operators once, then jdft_apply_H_host_resident (+ jdft_overlap_host_resident on the block it uploaded) per step"}
         del host, Vp, Dp
 
     # SURVEY 8(f) rank 1 operations on the same inputs (k-point 0): density of all bands, subspace Hamiltonian C^+ (H C)
@@ -566,7 +566,7 @@ def extra_ops(jd, torch, t_op, k, V, S, nb, nproj, cfg, R, Ecut, local):
     ms_h = t_op(lambda: jd.jdft_apply_H(gb, V, P, Qb, C, k["HC"]))
     nG = k["info"]["nG"]
     out["apply_O_us_blockQ"] = {"ms": ms_o, "TFLOP/s": 16.0 * nb * nproj * nG / (ms_o * 1e-3) / 1e12}
-    out["overlap_us_blockQ"] = {"ms": ms_m, "TFLOP/s": (8.0 * (nb * (nb + 1) // 2) * nG + 16.0 * nb * nproj * nG) / (ms_m * 1e-3) / 1e12}
+    out["overlap_us_blockQ"] = {"ms": ms_m, "TFLOP/s": (8.0 * (nb * (nb + 1) // 2) * nG + 8.0 * nb * nproj * nG) / (ms_m * 1e-3) / 1e12}
     out["apply_H_blockD"] = {"ms": ms_h, "band_apps_per_s": nb / (ms_h * 1e-3)}
     # Listing 1 on real fields: the density-cutoff basis (4 x Ecut, Gamma) as the scalar-field basis, 16 fields
     gs = jd.jdft_basis_create(R, [0.0, 0.0, 0.0], 4.0 * Ecut, S, device=local)

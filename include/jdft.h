@@ -185,6 +185,10 @@ int jdft_overlap_host(jdft_basis *b, const double *C1_host, int nb1, const doubl
 int jdft_host_set_operators(jdft_basis *b, const double *Vloc_host, const double *P_host, int nproj,
                             const double *D_host, int D_mode);
 int jdft_apply_H_host_resident(jdft_basis *b, const double *C_host, int nb, double *HC_host);
+/* M = C^+ O C (column-major nb x nb, HOST) of the band block the last jdft_apply_H_host / _resident call uploaded: H C and
+ * the overlap of the same bands are needed together in every SCF step, so C is not uploaded a second time.  JDFT_EINVAL
+ * if no such block of nb bands is on the device (any other *_host call in between invalidates it).                  */
+int jdft_overlap_host_resident(jdft_basis *b, int nb, double *M_host);
 
 /* ---- diagnostics ---------------------------------------------------------------------------------- */
 const char *jdft_last_error(void);

@@ -19,7 +19,7 @@ EXPORTS = [
     "jdft_basis_create", "jdft_basis_destroy", "jdft_basis_info", "jdft_basis_structure", "jdft_basis_export",
     "jdft_basis_device_maps", "jdft_workspace_bytes", "jdft_set_workspace", "jdft_set_option",
     "jdft_apply_I", "jdft_apply_Idag", "jdft_apply_J", "jdft_apply_L", "jdft_apply_O", "jdft_apply_Vnl",
-    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_pcm_hessian_real", "jdft_apply_H_host", "jdft_overlap_host", "jdft_host_set_operators", "jdft_apply_H_host_resident",
+    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_pcm_hessian_real", "jdft_apply_H_host", "jdft_overlap_host", "jdft_host_set_operators", "jdft_apply_H_host_resident", "jdft_overlap_host_resident",
     "jdft_last_error", "jdft_launch_count", "jdft_profile_read", "jdft_version",
 ]
 
@@ -64,6 +64,7 @@ def _load():
     L.jdft_overlap_host.argtypes = [vp, vp, ci, vp, ci, vp]
     L.jdft_host_set_operators.argtypes = [vp, vp, vp, ci, vp, ci]
     L.jdft_apply_H_host_resident.argtypes = [vp, vp, ci, vp]
+    L.jdft_overlap_host_resident.argtypes = [vp, ci, vp]
     L.jdft_last_error.restype = ctypes.c_char_p
     L.jdft_launch_count.argtypes = [ci]
     L.jdft_launch_count.restype = i64
@@ -410,6 +411,12 @@ def jdft_apply_H_host_resident(basis, C, HC):
     _chk(_lib.jdft_apply_H_host_resident(basis._h, _host(C, torch.complex128, "C"), int(C.shape[0]),
                                          _host(HC, torch.complex128, "HC")))
     return HC
+
+
+def jdft_overlap_host_resident(basis, M):
+    """C^+ O C of the bands the last jdft_apply_H_host[_resident] call uploaded (no second upload); M: HOST [nb, nb]."""
+    _chk(_lib.jdft_overlap_host_resident(basis._h, int(M.shape[0]), _host(M, torch.complex128, "M")))
+    return M.t()
 
 
 def jdft_overlap_host(basis, C1, C2, M):

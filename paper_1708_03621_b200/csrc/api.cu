@@ -299,6 +299,7 @@ int host_H_pipeline(jdft_basis *b, bool upload_ops, const double *Vh, const doub
     const size_t cb = (size_t)nb * nG * 16;
     void *dCv, *dHCv, *dW;
     int rc;
+    b->h_C_nb = 0;
     if ((rc = host_buf(b, 0, cb, &dCv)) || (rc = host_buf(b, 1, cb, &dHCv))) return rc;
     double *dC = (double *)dCv, *dHC = (double *)dHCv;
     int nchunk = (nb + 127) / 128;                       // chunks of <= 128 bands, at most 8 of them
@@ -368,6 +369,7 @@ int host_H_pipeline(jdft_basis *b, bool upload_ops, const double *Vh, const doub
     if (e1 != cudaSuccess) return jdft_cuda_fail(e1, who);
     if (e2 != cudaSuccess) return jdft_cuda_fail(e2, who);
     if (e3 != cudaSuccess) return jdft_cuda_fail(e3, who);
+    b->h_C_nb = nb;   // the band block stays on the device (hb[0]) for jdft_overlap_host_resident
     return JDFT_OK;
 }
 
@@ -433,6 +435,7 @@ extern "C" int jdft_overlap_host(jdft_basis *b, const double *C1, int nb1, const
     if (nb1 == 0 || nb2 == 0) return JDFT_OK;
     if (!C1 || !C2 || !M) return jdft_fail(JDFT_EINVAL, "overlap_host: null pointer");
     JDFT_CUDA(cudaSetDevice(b->device));
+    b->h_C_nb = 0;
     const bool same = C1 == C2 && nb1 == nb2;   // one upload; the device call then takes the Hermitian-triangle path
     const size_t b1 = (size_t)nb1 * b->nG * 16, b2 = (size_t)nb2 * b->nG * 16, mb = (size_t)nb1 * nb2 * 16;
     void *d1, *d2, *dM, *dW;
@@ -454,6 +457,37 @@ extern "C" int jdft_overlap_host(jdft_basis *b, const double *C1, int nb1, const
     if (e == cudaSuccess && !same) e = cudaMemcpyAsync(d2, C2, b2, cudaMemcpyHostToDevice, st);
     rc = e == cudaSuccess ? jdft_overlap(b, (const double *)d1, nb1, (const double *)d2, nb2, (double *)dM, st)
                           : jdft_cuda_fail(e, "overlap_host H2D");
+    b->ws = saved_ws;
+    b->ws_bytes = saved_bytes;
+    if (rc) { cudaStreamSynchronize(st); return rc; }
+    JDFT_CUDA(cudaMemcpyAsync(M, dM, mb, cudaMemcpyDeviceToHost, st));
+    JDFT_CUDA(cudaStreamSynchronize(st));
+    return JDFT_OK;
+}
+
+// M = C^+ O C of the band block that the last jdft_apply_H_host / jdft_apply_H_host_resident call left on the device:
+// H C and the overlap of the same bands are needed together in every SCF / minimiser step, so the second
+// upload of C is skipped; only the nb x nb result crosses PCIe.
+extern "C" int jdft_overlap_host_resident(jdft_basis *b, int nb, double *M) {
+    if (!b) return jdft_fail(JDFT_EINVAL, "overlap_host_resident: null basis");
+    if (nb <= 0 || !M) return jdft_fail(JDFT_EINVAL, "overlap_host_resident: bad size or null pointer");
+    if (b->h_C_nb != nb) return jdft_fail(JDFT_EINVAL, "overlap_host_resident: the last apply_H_host call left %d bands on the device, not %d", b->h_C_nb, nb);
+    JDFT_CUDA(cudaSetDevice(b->device));
+    const size_t mb = (size_t)nb * nb * 16;
+    void *dM, *dW;
+    int rc;
+    if ((rc = host_buf(b, 6, mb, &dM))) return rc;
+    if ((rc = host_streams(b, 1))) return rc;
+    void *saved_ws = b->ws;
+    size_t saved_bytes = b->ws_bytes;
+    if (!b->ws) {
+        size_t need = jdft_workspace_bytes(b, 1, nb);
+        if ((rc = host_buf(b, 5, need, &dW))) return rc;
+        b->ws = dW;
+        b->ws_bytes = need;
+    }
+    cudaStream_t st = b->hs[1];
+    rc = jdft_overlap(b, (const double *)b->hb[0], nb, (const double *)b->hb[0], nb, (double *)dM, st);
     b->ws = saved_ws;
     b->ws_bytes = saved_bytes;
     if (rc) { cudaStreamSynchronize(st); return rc; }

@@ -162,7 +162,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     for (int i = 0; i < 8; i++) { b->hb[i] = nullptr; b->hb_bytes[i] = 0; }
     for (int i = 0; i < 3; i++) b->hs[i] = nullptr;
     b->opt_graph = -1; b->gstream = nullptr;
-    b->h_ops_set = 0; b->h_nproj = 0; b->h_D_mode = 0;
+    b->h_ops_set = 0; b->h_nproj = 0; b->h_D_mode = 0; b->h_C_nb = 0;
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
     b->opt_profile_kernel = 0; b->prof_used = 0;
     b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_gemm3m = 1; b->opt_tma = 0; b->opt_gemm_tma = 0; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;

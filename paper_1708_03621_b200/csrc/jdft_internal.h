@@ -76,6 +76,7 @@ struct jdft_basis {
     cudaStream_t gstream;                     // capture stream
     cudaStream_t hs[3];                       // H2D, compute and D2H streams of the *_host pipeline (created on first use)
     std::vector<cudaEvent_t> hev;
+    int h_C_nb;                               // bands of the last host call still valid in hb[0] (0: none)
     int h_ops_set, h_nproj, h_D_mode;         // resident operators of jdft_host_set_operators (in hb[2..4])
 };
 

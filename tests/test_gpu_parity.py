@@ -230,6 +230,12 @@ def test_host_pipeline_chunks_and_resident_operators(ref, jd):
     HC2 = torch.empty(c.C.shape, dtype=torch.complex128).pin_memory()
     jd.jdft_apply_H_host_resident(c.gb, Ct, HC2)
     assert rel_err_per_band(HC2.numpy(), want) <= TOL
+    # the overlap of the block that call left on the device (no second upload)
+    Mh = torch.empty((c.nb, c.nb), dtype=torch.complex128).pin_memory()
+    gotM = jd.jdft_overlap_host_resident(c.gb, Mh).numpy()
+    assert rel_err_per_band(gotM.T, c.rb.overlap(c.C, c.C).T) <= TOL
+    with pytest.raises(jd.JdftError):                       # a different band count is refused
+        jd.jdft_overlap_host_resident(c.gb, torch.empty((c.nb - 1, c.nb - 1), dtype=torch.complex128))
     rng = np.random.default_rng(3)
     n = c.P.shape[0]
     A = rng.standard_normal((n // 4, 4, 4)) + 1j * rng.standard_normal((n // 4, 4, 4))

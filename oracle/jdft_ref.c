@@ -32,7 +32,8 @@
  *   H          H C = -1/2 L C + I^+( Vloc .* (I C) ) + P D P^+ C  (BASELINE.json north_star)
  *   overlap    M = C1^+ O C2 = Omega C1^+ C2, column-major nb1 x nb2
  *
- * Algorithm (deliberately naive): a zero-filled full box per band; three
+ * Algorithm (deliberately naive): the basis by a plain sweep of 2 S_d + 1 integers per axis (no ellipsoid
+ * geometry) plus a literal collision check; a zero-filled full box per band; three
  * un-pruned passes of a recursive mixed-radix decimation-in-time 1-D FFT (any
  * prime factor; O(p) butterflies written as the plain DFT sum), pencils copied
  * to a contiguous buffer; separate V multiply, gather, kinetic passes; GEMMs
@@ -43,7 +44,11 @@
  * J I = 1; I J idempotent; Parseval; adjointness; cos-potential closed form
  * (sign + wrap); translation covariance; L/ke closed forms; Omega values;
  * plane-wave eigenvalue ke + V0; Hermiticity; Vnl vs dense P D P^+, rank-1,
- * D = 0; basis vs exact counts, inversion symmetry, continuum count.
+ * D = 0; basis vs exact counts, inversion symmetry, continuum count; block-diagonal D and the ultrasoft
+ * O_us / overlap_us vs dense nG x nG matrices, positivity, Q = 0; density / subspace vs explicit matrices;
+ * gradient / divergence / Listing-1 hessian vs finite differences and explicit matrices; the real-field
+ * (half-sphere) hessian vs the complex path, realness of I, inversion symmetry of the order.
+ * No function of this file is "parity unpinned".
  * Unpinned by the paper: the CHOICE of conventions (readings 2-11); see DESIGN.md.
  *
  * Layouts: complex128 = double[2] (re, im) interleaved.  C is [nb][nG]

@@ -759,3 +759,60 @@ def test_pcm_hessian_real_fields(ref, jd, cfg_id, nb):
         with pytest.raises(jd.JdftError) as e:
             jd.jdft_pcm_hessian_real(gk, dev(eps.reshape(-1)), torch.zeros((1, (gk.nG + 1) // 2), dtype=torch.complex128, device="cuda"))
         assert e.value.code == jd.JDFT_EINVAL
+
+
+# ------------------------------------------------------------------------------------------ degenerate cases
+
+@pytest.mark.parametrize("S,L,k,Ecut", [((32, 32, 32), 10.0, (0.0, 0.0, 0.0), 0.1),      # nG = 1: only G = 0
+                                        ((32, 32, 32), 10.0, (0.0, 0.0, 0.0), 0.25),     # nG = 7: origin + 6 neighbours
+                                        ((8, 8, 8), 10.0, (0.0, 0.0, 0.0), 3.1),         # m = -3..3 on every axis: extent 7 of 8, the collision limit
+                                        ((12, 15, 20), 9.0, (0.5, 0.5, 0.5), 1.0)])      # k at the zone corner: asymmetric extents
+def test_degenerate_spheres_single_band_single_projector(ref, jd, S, L, k, Ecut):
+    """The smallest spheres (one plane wave; the origin and its six neighbours), a sphere that fills the box up to the
+    collision limit, one band and one projector: H, Vnl, I / J, overlap, density against the oracle."""
+    R = np.diag([L, L, L])
+    rb = ref.RefBasis(R, k, Ecut, S)
+    gb = jd.jdft_basis_create(R, k, Ecut, S)
+    iG, index, _ = jd.jdft_basis_export(gb)
+    assert np.array_equal(iG, rb.iG) and np.array_equal(index, rb.index)
+    if Ecut == 0.1:
+        assert rb.nG == 1
+    if Ecut == 0.25:
+        assert rb.nG == 7
+    rng = np.random.default_rng(int(100 * Ecut) + S[0])
+    C = rng.standard_normal((1, rb.nG)) + 1j * rng.standard_normal((1, rb.nG))
+    P = rng.standard_normal((1, rb.nG)) + 1j * rng.standard_normal((1, rb.nG))
+    D = np.array([0.7])
+    V = rng.standard_normal(S) * (rb.volume / rb.N)
+    jd.jdft_alloc_workspace(gb, 1, 1)
+    args = (dev(V.reshape(-1)), dev(P), dev(D), dev(C))
+    assert rel_err_per_band(jd.jdft_apply_H(gb, *args).cpu().numpy(), rb.apply_H(V, P, D, C)) <= TOL
+    assert rel_err_per_band(jd.jdft_apply_Vnl(gb, dev(P), dev(D), dev(C)).cpu().numpy(), rb.apply_Vnl(P, D, C)) <= TOL
+    psi = jd.jdft_apply_I(gb, dev(C))
+    assert rel_err_per_band(psi.cpu().numpy(), rb.apply_I(C)) <= TOL
+    assert rel_err_per_band(jd.jdft_apply_J(gb, psi).cpu().numpy(), C) <= 1e-13
+    M = jd.jdft_overlap(gb, dev(C), dev(C)).cpu().numpy()
+    assert abs(M[0, 0] - rb.overlap(C, C)[0, 0]) <= TOL * abs(M[0, 0])
+    n = jd.jdft_density(gb, dev(C), dev(np.array([1.3]))).cpu().numpy()
+    want_n = rb.density(C, np.array([1.3]))
+    assert np.linalg.norm(n - want_n) <= TOL * np.linalg.norm(want_n)
+
+
+def test_plane_wave_eigenvalue_on_the_gpu(ref, jd):
+    """north_star's closed form directly on the CUDA path: C = e_n, V_loc = (Omega/N) V0, no projectors =>
+    HC = (ke[n] + V0) Omega e_n and every other entry is zero to rounding."""
+    R, kpts, Ecut, S = workloads.lattice(102)
+    gb = jd.jdft_basis_create(R, kpts[0], Ecut, S)
+    _, _, ke = jd.jdft_basis_export(gb)
+    jd.jdft_alloc_workspace(gb, 3, 3)
+    V0 = -0.37
+    V = torch.full((gb.N,), V0 * gb.volume / gb.N, dtype=torch.float64, device="cuda")
+    sel = [0, gb.nG // 3, gb.nG - 1]
+    C = torch.zeros((3, gb.nG), dtype=torch.complex128, device="cuda")
+    for i, n0 in enumerate(sel):
+        C[i, n0] = 1.0 - 0.5j
+    HC = jd.jdft_apply_H(gb, V, None, None, C).cpu().numpy()
+    for i, n0 in enumerate(sel):
+        want = np.zeros(gb.nG, complex)
+        want[n0] = (ke[n0] + V0) * gb.volume * (1.0 - 0.5j)
+        assert np.max(np.abs(HC[i] - want)) <= 1e-13 * gb.volume * max(1.0, ke[n0])

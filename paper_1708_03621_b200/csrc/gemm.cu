@@ -334,13 +334,17 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
     const int row0 = blockIdx.x * BM;
     const int64_t n0 = (int64_t)blockIdx.y * BN_;
     const int nkt = (K + BK - 1) / BK;
-    if (Add) {   // pull the tile the epilogue adds to towards L2 while the main loop runs
+    // pull the tile the epilogue adds to towards L2 shortly before it is needed (PF_AHEAD k-tiles before the end: early
+    // enough to cover the HBM latency, late enough that the lines are still resident -- a CTA lives for ~140 us at K = 864)
+    constexpr int PF_AHEAD = 12;
+    auto prefetch_out = [&]() {
         for (int e = tid; e < BM * ((BN_ * 16 + 127) / 128); e += NTHREADS) {
             const int r = e / ((BN_ * 16 + 127) / 128), seg = e % ((BN_ * 16 + 127) / 128);
             if (row0 + r < Rn && n0 + seg * 8 < Nn)
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(Add + (size_t)(row0 + r) * Nn + n0 + seg * 8));
         }
-    }
+    };
+    if (Add && (!M3 || nkt <= PF_AHEAD)) prefetch_out();   // short K (4M kernel): at the start
 
     double cr[MTL][NTL][2], ci[MTL][NTL][2], c3[M3 ? MTL : 1][M3 ? NTL : 1][2];   // 3M: k1, k2, k3 (see k_gemm_dotk)
 #pragma unroll
@@ -374,6 +378,7 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
     for (int kt = 0; kt < nkt; kt++) {
         cp_async_wait<ST - 2>();
         __syncthreads();
+        if (M3 && Add && kt == nkt - PF_AHEAD) prefetch_out();
         {
             const int nx = kt + ST - 1;
             if (nx < nkt) {

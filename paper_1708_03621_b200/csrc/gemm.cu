@@ -1,12 +1,17 @@
 // Complex FP64 GEMMs on the FP64 tensor pipe (DMMA, mma.sync.m8n8k4.f64) for the nonlocal projectors and the
 // subspace overlap.  tcgen05 has no FP64 kind, so on sm_100a the FP64 tensor path is
-// the warp-level DMMA; one complex MAC tile = four real DMMAs (Cr += ArBr -/+ AiBi, Ci += ArBi +/- AiBr).
+// the warp-level DMMA; one complex MAC tile = four real DMMAs (Cr += ArBr -/+ AiBi, Ci += ArBi +/- AiBr) in the 4M
+// kernels, THREE in the 3M (Karatsuba) kernels that serve the large contractions (see k_gemm_dotk below).
 //
 //   k_gemm_dotk   Out[r][c] = sum_k X[r][k] * conj?(Y[c][k])     both operands K-contiguous (K = nG), split-K with
 //                 a fixed-order reduction (deterministic, no atomics): P^+ C, C1^+ C2, and D.B for dense D
 //   k_gemm_expand Out[r][n] (+)= sum_j A[r][j] * Pm[j][n]        K = nproj, n contiguous: P (D P^+ C)
 //
-// Tiles: 64 x 64 per CTA, 4 warps of 32 x 32 (4 x 4 DMMA tiles of 8 x 8), BK = 8, 4-stage cp.async pipeline.
+//                 (epilogue: Out = A Pm + addscale Add, which serves HC += ..., and Omega C + ... of O_us)
+//   k_splitk_reduce[_block]  fixed-order split-K reduction with the scale, the real diagonal or the per-atom block D
+//
+// Tiles: 64 x 64 per CTA (4M), 4 warps of 32 x 32 (4 x 4 DMMA tiles of 8 x 8); 64 x 48 (3M: three accumulator sets);
+// BK = 8, 4-stage cp.async pipeline (6 stages in the 3M expand kernel).
 // Shared-memory layout of a K-contiguous operand: per group of 4 k, a dense [64 rows][4 k] block of c128
 // (64 B per row, so the 8 lanes of a quarter-warp read 128 contiguous bytes), blocks skewed by 64 B.
 #include <cstring>

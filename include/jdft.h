@@ -106,14 +106,20 @@ int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
 int jdft_set_option(jdft_basis *b, const char *key, int64_t value);
 
 /* ---- operators ------------------------------------------------------ */
-/* I: C [nb][nG] -> psi [nb][N]   (scatter + inverse 3-D FFT, unnormalised, sign +)                    */
+/* I ("the operators I and J Fourier transform from reciprocal to real space and vice versa (using Fast
+ * Fourier Transforms)"; rows a1 + a2; readings 2, 3, 8, 9): C [nb][nG] -> psi [nb][N], sphere -> box
+ * scatter + inverse 3-D FFT, unnormalised, sign +.                                                       */
 int jdft_apply_I(const jdft_basis *b, const double *C, int nb, double *psi, jdft_stream s);
-/* Idag: psi [nb][N] -> C [nb][nG] (forward 3-D FFT, sign -, + gather)                                 */
+/* Idag (the adjoint of I that H C needs, BASELINE.json north_star; row a4 + the gather of a5): psi [nb][N] ->
+ * C [nb][nG], forward 3-D FFT (sign -) + box -> sphere gather.  psi may hold components outside the sphere.  */
 int jdft_apply_Idag(const jdft_basis *b, const double *psi, int nb, double *C, jdft_stream s);
-/* J = Idag / N                                                                                        */
+/* J (the inverse transform of I; reading 2): J = Idag / N, so J I = 1 on the sphere.     */
 int jdft_apply_J(const jdft_basis *b, const double *psi, int nb, double *C, jdft_stream s);
-/* L C = -2 Omega ke C ; O C = Omega C.  May run in place (out == C).                                  */
+/* L (gradient / divergence "apply in reciprocal space (where they are diagonal)", L = div grad;
+ * DESIGN.md readings 4, 6): L C = -Omega |G+k|^2 C = -2 Omega ke C.  May run in place (LC == C).               */
 int jdft_apply_L(const jdft_basis *b, const double *C, int nb, double *LC, jdft_stream s);
+/* O ("the integral is evaluated as a dot product with the overlap operator O", "diagonal in the
+ * plane-wave basis"; reading 4): O C = Omega C.  May run in place.                                  */
 int jdft_apply_O(const jdft_basis *b, const double *C, int nb, double *OC, jdft_stream s);
 /* Vnl: out (+)= P D P^+ C (PAPER.md:127 SpeciesInfo pseudopotentials).  P c128[nproj][nG];
  * D_mode 0: D = f64[nproj] real diagonal;  D_mode 1: D = c128[nproj][nproj] row-major Hermitian;
@@ -122,14 +128,16 @@ int jdft_apply_O(const jdft_basis *b, const double *C, int nb, double *OC, jdft_
  * The same three layouts are accepted wherever a D or Q is taken.  accumulate != 0 adds into out.              */
 int jdft_apply_Vnl(const jdft_basis *b, const double *P, int nproj, const double *D, int D_mode,
                    const double *C, int nb, double *out, int accumulate, jdft_stream s);
-/* projection alone: Bproj [nb][nproj] = (P^+ C)^T, i.e. Bproj[ib][j] = sum_n conj(P[j][n]) C[ib][n]   */
+/* projection alone (row a6): Bproj [nb][nproj] = (P^+ C)^T, i.e. Bproj[ib][j] = sum_n conj(P[j][n]) C[ib][n]    */
 int jdft_project(const jdft_basis *b, const double *P, int nproj, const double *C, int nb, double *Bproj,
                  jdft_stream s);
-/* H: HC = -1/2 L C + I^+ (Vloc .* I C) + P D P^+ C.  Vloc f64[N] is used exactly as passed (the caller
+/* H (BASELINE.json north_star; rows a1-a8 as one fused pipeline, the real-space psi never reaches HBM):
+ * HC = -1/2 L C + I^+ (Vloc .* I C) + P D P^+ C.  Vloc f64[N] is used exactly as passed (the caller
  * folds in the quadrature weight Omega/N; reading 5).  nproj == 0 skips the nonlocal term.  */
 int jdft_apply_H(const jdft_basis *b, const double *Vloc, const double *P, int nproj, const double *D,
                  int D_mode, const double *C, int nb, double *HC, jdft_stream s);
-/* overlap: M[a + nb1*bb] = Omega sum_n conj(C1[a][n]) C2[bb][n]  (column-major nb1 x nb2, c128)       */
+/* overlap (row a9; PAPER.md:76 integrals as dot(a, O b)): M[a + nb1*bb] = Omega sum_n conj(C1[a][n]) C2[bb][n]
+ * (column-major nb1 x nb2, c128).  C1 == C2 (same pointer) computes the Hermitian triangle only and mirrors it.  */
 int jdft_overlap(const jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M,
                  jdft_stream s);
 

@@ -83,3 +83,31 @@ def test_algorithmic_bytes_match_design_formula():
 def test_bench_help_renders():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--help"], capture_output=True, text=True, timeout=120)
     assert out.returncode == 0 and "--config" in out.stdout
+
+
+def test_committed_bench_line_has_every_contract_key():
+    """The line `python bench.py` printed on the B200 (committed under profiles/bench_r02/) carries every key of the
+    measurement contract: base keys, clocks, e2e with byte counts, gpu_launches, roofline, cpu_baseline."""
+    import json
+    path = os.path.join(ROOT, "profiles", "bench_r02", "default_run.txt")
+    line = [l for l in open(path) if l.startswith("{")][-1]
+    d = json.loads(line)
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert k in d, k
+    assert d["config"]["workload"] == "cfg5_bulk216_G_128^3" and d["dtype"] == "f64" and d["vs_baseline"] is None
+    assert d["n_gpus"] == 1 and d["warmup"] >= 3 and d["gpu_launches"] > 0
+    assert set(("sm_mhz", "sm_max_mhz", "reasons")) <= set(d["clocks"])
+    assert not set(d["clocks"]["reasons"]) & {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+    for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step"):
+        assert k in d["e2e"]
+    assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] > 0 and d["e2e"]["value"] < d["value"]
+    r = d["roofline"]
+    for k in ("bound", "achieved", "peak", "unit", "frac", "traffic"):
+        assert k in r
+    assert r["bound"] in ("hbm", "tensor", "alu") and r["traffic"] is not None
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) <= 1e-9
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and "sample" in c and c["unit"] == d["unit"]
+    # the value is units / time
+    assert abs(d["value"] - d["config"]["bands"] * d["config"]["kpoints"] / (d["ms_per_step"] * 1e-3)) <= 1e-6 * d["value"]

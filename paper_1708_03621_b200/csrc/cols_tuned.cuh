@@ -15,12 +15,14 @@
 namespace jcols {
 using namespace jfft;
 
-template <int LT>
+// REV (two-pass plans only): the radices in reversed order (128 = 16 x 8 instead of 8 x 16), so that the LAST pass is the
+// radix-8 one and can be output-pruned (K5) the way K1's first pass is input-pruned.
+template <int LT, bool REV = false>
 struct Cfg {
     using P = SpecPlan<LT>;
     static constexpr int NP = P::npass;
     static constexpr bool ok = NP == 2 || NP == 3;
-    static constexpr int R0 = P::r0, R1 = P::r1, R2 = P::r2;
+    static constexpr int R0 = (REV && NP == 2) ? P::r1 : P::r0, R1 = (REV && NP == 2) ? P::r0 : P::r1, R2 = P::r2;
     static constexpr int RL = NP == 3 ? R2 : R1;               // radix of the last pass
     static constexpr int T = NP == 3 ? 8 : 16;                  // pencils per CTA
     static constexpr int TP = T + 1;
@@ -29,7 +31,7 @@ struct Cfg {
     static constexpr int FIT = ok ? 65536 / (T * (LT / R0) / ((NP == 2 && LT / R0 == 2 * (LT / RL)) ? 2 : 1) * (RMAX >= 15 ? 80 : (RMAX >= 12 ? 72 : 40))) : 1;
     static constexpr int MINB_DEF = FIT < 1 ? 1 : (FIT > 6 ? 6 : FIT);
     // measured choices for the lengths of the five workloads (profiles/), the rule for the rest
-    static constexpr int MINB_INV = LT == 216 ? 5 : (LT == 128 ? 6 : MINB_DEF), MINB_FWD = LT == 216 ? 4 : (LT == 128 ? 6 : MINB_DEF);
+    static constexpr int MINB_INV = LT == 216 ? 5 : (LT == 128 ? 6 : MINB_DEF), MINB_FWD = REV ? 4 : (LT == 216 ? 4 : (LT == 128 ? 6 : MINB_DEF));
     static constexpr int NBL = ok ? LT / RL : 1;                // butterflies per pencil in the last pass
     static constexpr int NB0 = ok ? LT / R0 : 1;                // ... in the first pass
     // ONE swizzled tile [L][T]; the shared -> shared passes run in a single round (threads = their work items) and
@@ -128,7 +130,7 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tun
         // scatter the sphere runs of the nc columns (contiguous in n) into the tile; nothing else of it is read
         // (the sphere reads are issued four deep before the first dependent shared-memory store: their HBM latency was
         //  the largest single stall of the kernel in the ncu source page)
-        constexpr int U = F::NP == 3 ? 1 : 4;   // measured: pays at 128 (0.874 -> 0.847 ms) and 80, not at 216 (40 registers)
+        constexpr int U = F::NP == 3 ? 1 : 4;   // measured: pays at 128 (0.874 -> 0.847 ms at U = 4) and 80, not at 216 (40 registers)
         for (int e0 = tid; e0 < nend - nbeg; e0 += U * NT) {
             double2 v[U];
 #pragma unroll
@@ -200,22 +202,36 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tun
 
 // ------------------------------------------------------------------------------------------------ K5
 // out[b][n] = scale * (F_2 W1)[column of n][m2 of n]  (+ kin * ke[n] * C[b][n])
-template <int LT>
-__global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_FWD) k_cols_fwd_tuned(const double2 *__restrict__ tw, const int ncol,
+template <int SIGN>
+__device__ __forceinline__ void dft8_out0167_c(double2 (&a)[8]) {   // outputs 0, 1, 6, 7 of the length-8 DFT (a[2..5] undefined on exit)
+    const double2 s0 = cadd(a[0], a[4]), s1 = cadd(a[1], a[5]), s2 = cadd(a[2], a[6]), s3 = cadd(a[3], a[7]);
+    const double2 d0 = csub(a[0], a[4]), d1 = csub(a[1], a[5]), d2 = csub(a[2], a[6]), d3 = csub(a[3], a[7]);
+    const double2 j2 = mul_i<SIGN>(d2), j3 = mul_i<SIGN>(d3);
+    a[0] = cadd(cadd(s0, s2), cadd(s1, s3));
+    a[6] = csub(csub(s0, s2), mul_i<SIGN>(csub(s1, s3)));
+    a[1] = cadd(cadd(d0, j2), mul_w<SIGN, 1, 8>(cadd(d1, j3)));
+    a[7] = cadd(csub(d0, j2), mul_w<SIGN, 7, 8>(csub(d1, j3)));
+}
+
+// REV = true: reversed radix order with the radix-8 LAST pass pruned to outputs 0, 1, 6, 7 (rows [2 NBL, 6 NBL) hold no
+// sphere point, the gather never reads them); the launcher checks |m2| < 2 NBL.
+template <int LT, bool REV = false>
+__global__ void __launch_bounds__(Cfg<LT, REV>::NT, Cfg<LT, REV>::MINB_FWD) k_cols_fwd_tuned(const double2 *__restrict__ tw, const int ncol,
                                                                 const int64_t nG, const int *__restrict__ col_n0,
                                                                 const int *__restrict__ col_m2lo,
                                                                 const double2 *__restrict__ W1, const double scale,
                                                                 const double kin, const double *__restrict__ ke,
                                                                 const double2 *__restrict__ C, double2 *__restrict__ outC) {
-    using F = Cfg<LT>;
+    using F = Cfg<LT, REV>;
     constexpr int T = F::T, TP = F::TP, NT = F::NT, L = LT, R0 = F::R0, R1 = F::R1, RL = F::RL, NBL = F::NBL, NB0 = F::NB0;
+    static_assert(!REV || (F::NP == 2 && RL == 8), "the reversed plan ends with the radix-8 pass");
     extern __shared__ double2 smem[];
     double2 *X = smem;
     __shared__ int s_n0[T + 1], s_m2w[T];
     const int tid = threadIdx.x, c0 = blockIdx.x * T, b = blockIdx.y;
     const int nc = min(T, ncol - c0);
-    if (tid <= T) s_n0[tid] = col_n0[min(c0 + tid, ncol)];
-    if (tid < T) s_m2w[tid] = wrap_row(col_m2lo[min(c0 + tid, ncol - 1)], L);
+    for (int i = tid; i <= T; i += NT) s_n0[i] = col_n0[min(c0 + i, ncol)];
+    for (int i = tid; i < T; i += NT) s_m2w[i] = wrap_row(col_m2lo[min(c0 + i, ncol - 1)], L);
     if (kin != 0.0 && LT == 128) {   // measured: 1.126 -> 1.116 ms at 128; slower at 80 and 216
         // the gather at the end reads C and ke of this CTA's sphere run (contiguous in n) straight from HBM, and nothing
         // hides that latency there (ncu: 45 % of the warp samples on long-scoreboard stalls): ask L2 for those lines now,
@@ -250,9 +266,13 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_FWD) k_cols_fwd_tun
             double2 a[RL];
 #pragma unroll
             for (int k = 0; k < RL; k++) a[k] = X[F::sw(bf + k * NBL, t)];
-            Dft<RL, -1>::run(a);
+            if constexpr (REV) dft8_out0167_c<-1>(a);
+            else Dft<RL, -1>::run(a);
 #pragma unroll
-            for (int j = 0; j < RL; j++) X[F::sw(bf + NBL * j, t)] = a[j];
+            for (int j = 0; j < RL; j++) {
+                if (REV && j >= 2 && j < 6) continue;
+                X[F::sw(bf + NBL * j, t)] = a[j];
+            }
         }
     }
     __syncthreads();

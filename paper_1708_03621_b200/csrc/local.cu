@@ -1164,10 +1164,20 @@ int launch_cols_fwd(const jdft_basis *b, const double2 *W1, int nbt, double scal
     SPEC_SWITCH(L, b->opt_force_generic, {
         if constexpr (jcols::Cfg<LT>::ok) {
             using F = jcols::Cfg<LT>;
-            JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT>, F::smem, b->device));
-            dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
-            jcols::k_cols_fwd_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
-                                                               scale, kin, b->d_ke, C, out);
+            using FR = jcols::Cfg<LT, true>;
+            // reversed plan (16, 8) with the radix-8 last pass pruned, when no sphere point has |m2| >= 2 (L / 8); measured:
+            // 1.116 -> 0.949 ms at 128 (0.78 -> 0.91 of the HBM roofline), no gain at 80 = 8 x 10 (kept on the forward plan)
+            if (F::NP == 2 && F::R0 == 8 && F::R1 == 16 && b->opt_prune && b->mmin[2] > -2 * (LT / 8) && b->mmax[2] < 2 * (LT / 8)) {
+                JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT, F::NP == 2 && F::R0 == 8 && F::R1 == 16>, FR::smem, b->device));
+                dim3 g2((b->ncol + FR::T - 1) / FR::T, nbt);
+                jcols::k_cols_fwd_tuned<LT, F::NP == 2 && F::R0 == 8 && F::R1 == 16><<<g2, FR::NT, FR::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
+                                                                   scale, kin, b->d_ke, C, out);
+            } else {
+                JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT>, F::smem, b->device));
+                dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
+                jcols::k_cols_fwd_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
+                                                                   scale, kin, b->d_ke, C, out);
+            }
         } else {
             JDFT_CUDA(ensure_smem(k_cols_fwd<LT>, smem, b->device));
             k_cols_fwd<LT><<<grid, ColsNT<LT>::v, smem, st>>>(b->plan[2], b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,

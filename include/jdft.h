@@ -141,6 +141,17 @@ int jdft_apply_H(const jdft_basis *b, const double *Vloc, const double *P, int n
 int jdft_overlap(const jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M,
                  jdft_stream s);
 
+/* overlap without any allocation or workspace (same result as jdft_overlap): for callers that cannot call cudaMalloc or
+ * hand over a workspace -- code under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  The
+ * split-K partials of the GEMM live in a 16 MiB file-scope static device array inside the library (held by every GPU that
+ * loads the library until the process exits), so the call allocates nothing and ignores the basis' workspace.
+ * LIMIT: nb1 * nb2 <= 65 536 entries (e.g. 256 x 256); larger sizes return JDFT_EINVAL with a message.  All calls on a
+ * device share the array (it keeps the last call's contents; nothing needs clearing): calls that overlap on the GPU
+ * (different streams) race -- use one stream at a time per device.  The first call per device resolves the array's
+ * address and should be made outside graph capture.                                                                   */
+int jdft_overlap_noalloc(const jdft_basis *b, const double *C1, int nb1, const double *C2, int nb2, double *M,
+                         jdft_stream s);
+
 /* ---- ultrasoft pseudopotentials ("norm-conserving and ultrasoft pseudopotentials",
  * PAPER.md:166-169 Listing 2 runs on the GBRV ultrasoft library; reading 24) ------------------------------
  * generalised overlap operator   O_us C = Omega (C + P Q P^+ C),   Q in the layouts of D (Q_mode as D_mode);

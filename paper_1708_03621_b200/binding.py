@@ -19,7 +19,7 @@ EXPORTS = [
     "jdft_basis_create", "jdft_basis_destroy", "jdft_basis_info", "jdft_basis_structure", "jdft_basis_export",
     "jdft_basis_device_maps", "jdft_workspace_bytes", "jdft_set_workspace", "jdft_set_option",
     "jdft_apply_I", "jdft_apply_Idag", "jdft_apply_J", "jdft_apply_L", "jdft_apply_O", "jdft_apply_Vnl",
-    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_pcm_hessian_real", "jdft_apply_H_host", "jdft_overlap_host", "jdft_host_set_operators", "jdft_apply_H_host_resident", "jdft_overlap_host_resident",
+    "jdft_project", "jdft_apply_H", "jdft_overlap", "jdft_overlap_noalloc", "jdft_apply_O_us", "jdft_overlap_us", "jdft_subspace", "jdft_density", "jdft_gradient", "jdft_divergence", "jdft_pcm_hessian", "jdft_pcm_hessian_real", "jdft_apply_H_host", "jdft_overlap_host", "jdft_host_set_operators", "jdft_apply_H_host_resident", "jdft_overlap_host_resident",
     "jdft_last_error", "jdft_launch_count", "jdft_profile_read", "jdft_version",
 ]
 
@@ -53,6 +53,7 @@ def _load():
     L.jdft_apply_H.argtypes = [vp, vp, vp, ci, vp, ci, vp, ci, vp, vp]
     L.jdft_overlap.argtypes = [vp, vp, ci, vp, ci, vp, vp]
     L.jdft_subspace.argtypes = [vp, vp, ci, vp, ci, vp, vp]
+    L.jdft_overlap_noalloc.argtypes = [vp, vp, ci, vp, ci, vp, vp]
     L.jdft_apply_O_us.argtypes = [vp, vp, ci, vp, ci, vp, ci, vp, vp]
     L.jdft_overlap_us.argtypes = [vp, vp, ci, vp, ci, vp, ci, vp, ci, vp, vp]
     L.jdft_density.argtypes = [vp, vp, ci, vp, vp, ci, vp]
@@ -276,6 +277,17 @@ def jdft_overlap(basis, C1, C2, M=None):
         M = torch.empty((nb2, nb1), dtype=torch.complex128, device=C1.device)  # column-major nb1 x nb2
     _chk(_lib.jdft_overlap(basis._h, _dev(C1, torch.complex128, "C1"), nb1, _dev(C2, torch.complex128, "C2"), nb2,
                            _dev(M, torch.complex128, "M"), _stream()))
+    return M.t()
+
+
+def jdft_overlap_noalloc(basis, C1, C2, M):
+    """jdft_overlap with the split-K scratch in the library's static 16 MiB device array: no allocation, no workspace;
+    nb1 * nb2 <= 65536.  M: caller-provided CUDA complex128 [nb2, nb1] (column-major nb1 x nb2); returns the view M[a, b]."""
+    nb1, nb2 = _bands(C1, basis, "C1"), _bands(C2, basis, "C2")
+    if tuple(M.shape) != (nb2, nb1):
+        raise ValueError("M must have shape [nb2, nb1]")
+    _chk(_lib.jdft_overlap_noalloc(basis._h, _dev(C1, torch.complex128, "C1"), nb1, _dev(C2, torch.complex128, "C2"), nb2,
+                                   _dev(M, torch.complex128, "M"), _stream()))
     return M.t()
 
 

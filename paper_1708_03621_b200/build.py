@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libjdft_b200.so")
 PEAK_TOOL = os.path.join(HERE, "fp64_peak")  # micro-benchmark binary bench.py runs for the FP64 roofline peak
-SOURCES = ["basis.cu", "local.cu", "gemm.cu", "api.cu"]
+SOURCES = ["basis.cu", "local.cu", "gemm.cu", "api.cu", "noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "jdft_internal.h"), os.path.join(CSRC, "fft.cuh"), os.path.join(CSRC, "cols_tuned.cuh"), os.path.join(CSRC, "planes_tma.cuh"), os.path.join(CSRC, "tma.cuh"),
            os.path.join(HERE, "..", "include", "jdft.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

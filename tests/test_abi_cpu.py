@@ -99,6 +99,8 @@ def test_null_and_bad_arguments_return_status_codes_without_a_device(lib):
     assert lib.jdft_apply_H_host_resident(None, None, 1, None) == EINVAL
     lib.jdft_overlap_host_resident.argtypes = [vp, ctypes.c_int, vp]
     assert lib.jdft_overlap_host_resident(None, 1, None) == EINVAL
+    lib.jdft_overlap_noalloc.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_int, vp, vp]
+    assert lib.jdft_overlap_noalloc(None, None, 1, None, 1, None, None) == EINVAL
     lib.jdft_version.restype = ctypes.c_char_p
     assert lib.jdft_version().startswith(b"jdft-b200")
 

@@ -210,3 +210,51 @@ def test_full_pcm_hessian_scalar_field_basis(ref, jd):
     e0 = 78.4
     got0 = jd.jdft_pcm_hessian(gb, dev(np.full(S, e0).reshape(-1)), dev(phi)).cpu().numpy()
     assert rel_rows(got0, (e0 / (4 * np.pi)) * (2.0 * ke)[None, :] * phi) <= 1e-12
+
+
+def test_full_ultrasoft_and_block_D(full, jd):
+    """SURVEY 8(f) rank 2 at full size (configs 2, 3, 5; one k-point of config 4): per-atom blocks of n_lm x n_lm (4 x 4, or
+    9 x 9 at config 3) for D in apply_H / apply_Vnl and for Q in apply_O_us / overlap_us.  The GPU processes ALL bands in
+    one call; the oracle checks 24 of them (head, tail and both sides of every batch boundary) band by band, and the
+    generalised overlap on 16 columns against all nb rows."""
+    if full.cfg_id == 4 and full.ik != 0:
+        pytest.skip("same shapes as k-point 0")
+    nblk = workloads.get_config(full.cfg_id)["n_lm"]
+    nproj = full.P.shape[0]
+    rng = np.random.default_rng(400 + full.cfg_id)
+    A = rng.standard_normal((nproj // nblk, nblk, nblk)) + 1j * rng.standard_normal((nproj // nblk, nblk, nblk))
+    Db = np.ascontiguousarray(A + A.conj().transpose(0, 2, 1))
+    Qb = np.ascontiguousarray(0.05 * (A @ A.conj().transpose(0, 2, 1)))
+    sub = full.subset[:24]
+    Cs = full.C[sub]
+    dDb, dQb = dev(Db), dev(Qb)
+    got = jd.jdft_apply_Vnl(full.gb, full.dP, dDb, full.dC)[sub].cpu().numpy()
+    assert rel_rows(got, full.rb.apply_Vnl(full.P, Db, Cs)) <= TOL
+    got = jd.jdft_apply_H(full.gb, full.dV, full.dP, dDb, full.dC)[sub].cpu().numpy()
+    assert rel_rows(got, full.rb.apply_H(full.V, full.P, Db, Cs)) <= TOL
+    got = jd.jdft_apply_O_us(full.gb, full.dP, dQb, full.dC)[sub].cpu().numpy()
+    assert rel_rows(got, full.rb.apply_O_us(full.P, Qb, Cs)) <= TOL
+    cols = sub[:16]
+    M = jd.jdft_overlap_us(full.gb, full.dP, dQb, full.dC, full.dC).cpu().numpy()      # same array: one projection, triangle overlap
+    want = full.rb.overlap_us(full.P, Qb, full.C, full.C[cols])                         # [nb, 16]
+    assert rel_rows(M[:, cols].T, want.T) <= TOL
+    assert np.max(np.abs(M - M.conj().T)) <= 1e-12 * np.max(np.abs(M))
+    C2 = dev(np.ascontiguousarray(full.C[cols] * (1.0 + 0.5j)))
+    M2 = jd.jdft_overlap_us(full.gb, full.dP, dQb, full.dC, C2).cpu().numpy()           # distinct operands
+    assert rel_rows(M2.T, (want * (1.0 + 0.5j)).T) <= TOL
+
+
+def test_full_pcm_hessian_real_fields(ref, jd):
+    """Listing 1 on REAL fields in half-sphere storage on the density-cutoff basis of the config-2 box (nG = 191 471): 4
+    fields (3 x 4 = 12 components -> 6 complex transforms) against the oracle's real-field function."""
+    R, _, Ecut, S = workloads.lattice(2)
+    k = [0.0, 0.0, 0.0]
+    rb = ref.RefBasis(R, k, 4 * Ecut, S)
+    gb = jd.jdft_basis_create(R, k, 4 * Ecut, S)
+    rng = np.random.default_rng(131)
+    nf, nGh = 4, (rb.nG + 1) // 2
+    ph = rng.standard_normal((nf, nGh)) + 1j * rng.standard_normal((nf, nGh))
+    eps = 1.0 + 78.0 * rng.random(S)
+    jd.jdft_set_workspace(gb, torch.empty(jd.jdft_workspace_bytes(gb, 3 * nf, 0) + 48 * nf * gb.nG, dtype=torch.uint8, device="cuda"))
+    got = jd.jdft_pcm_hessian_real(gb, dev(eps.reshape(-1)), dev(ph)).cpu().numpy()
+    assert rel_rows(got, rb.pcm_hessian_real(eps, ph)) <= TOL

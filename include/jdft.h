@@ -100,6 +100,7 @@ int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
  * 3M complex-product scheme, three tensor instructions per complex tile product instead of four),
  * "gemm_tma" (0/1, default 0: operand stages of the 3M GEMMs filled by cp.async.bulk.tensor instead of cp.async; measured
  * 5 % slower),
+ * "host_chunk" (bands per chunk of the jdft_apply_H_host pipeline; 0 = default 64),
  * "graph" (-1 auto / 0 off / 1 on: jdft_apply_H replays a captured CUDA graph when called again with the same pointers,
  * sizes and workspace; auto = calls of at most 4 Mi band x grid points, which are launch-bound),
  * "profile_kernel" (see diagnostics)                                                                    */

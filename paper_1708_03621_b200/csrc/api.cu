@@ -302,8 +302,8 @@ int host_H_pipeline(jdft_basis *b, bool upload_ops, const double *Vh, const doub
     b->h_C_nb = 0;
     if ((rc = host_buf(b, 0, cb, &dCv)) || (rc = host_buf(b, 1, cb, &dHCv))) return rc;
     double *dC = (double *)dCv, *dHC = (double *)dHCv;
-    int nchunk = (nb + 127) / 128;                       // chunks of <= 128 bands, at most 8 of them
-    if (nchunk > 8) nchunk = 8;
+    int nchunk = b->opt_host_chunk > 0 ? (int)((nb + b->opt_host_chunk - 1) / b->opt_host_chunk) : (nb + 63) / 64;   // chunks of <= 64 bands (option "host_chunk"; measured: config 5 73.3 / 70.5 / 91.0 ms at 128 / 64 / 32), at most 16
+    if (nchunk > 16) nchunk = 16;
     const int nbc = (nb + nchunk - 1) / nchunk;
     nchunk = (nb + nbc - 1) / nbc;
     if ((rc = host_streams(b, nchunk))) return rc;

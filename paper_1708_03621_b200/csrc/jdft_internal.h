@@ -59,6 +59,7 @@ struct jdft_basis {
     int64_t opt_overlap;
     int64_t opt_pair;                         // K3 with two pencils per thread where available ("planes_pair")
     int64_t opt_gemm3m;                       // GEMMs by the 3M complex-product scheme ("gemm_3m", default 1)
+    int64_t opt_host_chunk;                   // bands per chunk of the *_host pipeline ("host_chunk", 0 = 128)
     int64_t opt_gemm_tma;                     // operand stages of the 3M GEMMs filled by TMA ("gemm_tma")
     int64_t opt_tma;                          // K3 through TMA tensor-map loads / stores ("planes_tma")
     int64_t opt_prune;                        // K3 hybrid: radix-8 butterflies pruned to the occupied planes ("planes_prune")

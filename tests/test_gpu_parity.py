@@ -214,8 +214,8 @@ def test_host_variants(case, jd):
 
 
 def test_host_pipeline_chunks_and_resident_operators(ref, jd):
-    """jdft_apply_H_host pipelines band chunks over three streams; 300 bands of a small box span three chunks with a
-    ragged last one.  jdft_host_set_operators + jdft_apply_H_host_resident give the same result; a dense and a
+    """jdft_apply_H_host pipelines band chunks (64 bands by default) over three streams; 300 bands of a small box span five
+    chunks with a ragged last one.  jdft_host_set_operators + jdft_apply_H_host_resident give the same result; a dense and a
     block-diagonal D go through the same path; without a caller workspace the library allocates its own."""
     c = Case(ref, jd, 101, nb=300)
     want = c.rb.apply_H(c.V, c.P, c.D, c.C)

@@ -153,13 +153,15 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const __grid
         } else {
             cp_async_wait<ST - 2>();
             __syncthreads();
-            const int nx = kt + ST - 1;
-            if (nx < nkt) {
-                const int slot = nx % ST;
-                load_opk<BKT>(sX + slot * OPKT, X, K, Rn, row0, (kt0 + nx) * BKT, K, tid);
-                load_opk<BKT, BN_>(sY + slot * OPKT, Y, K, cend, col0, (kt0 + nx) * BKT, K, tid);
+            if constexpr (!M3) {   // 4M kernels: refill issued right away (the late issue below costs them registers)
+                const int nx = kt + ST - 1;
+                if (nx < nkt) {
+                    const int slot = nx % ST;
+                    load_opk<BKT>(sX + slot * OPKT, X, K, Rn, row0, (kt0 + nx) * BKT, K, tid);
+                    load_opk<BKT, BN_>(sY + slot * OPKT, Y, K, cend, col0, (kt0 + nx) * BKT, K, tid);
+                }
+                cp_async_commit();
             }
-            cp_async_commit();
         }
         const char *bx = sX + (kt % ST) * OPKT, *by = sY + (kt % ST) * OPKT;
 #pragma unroll
@@ -171,6 +173,19 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 1) k_gemm_dotk(const __grid
 #pragma unroll
             for (int j = 0; j < NTL; j++)
                 bq[j] = *reinterpret_cast<const double2 *>(by + kk * KBLK + (wc + 8 * j) * 64 + fo);
+            if constexpr (!TMA && M3) {
+                // the refill of the stage consumed in the previous k-tile is issued AFTER this k-tile's last fragment loads: a
+                // shared-memory load right behind the cp.async batch waited for it (ncu: 5 % of the warp samples)
+                if (kk == BKT / 4 - 1) {
+                    const int nx = kt + ST - 1;
+                    if (nx < nkt) {
+                        const int slot = nx % ST;
+                        load_opk<BKT>(sX + slot * OPKT, X, K, Rn, row0, (kt0 + nx) * BKT, K, tid);
+                        load_opk<BKT, BN_>(sY + slot * OPKT, Y, K, cend, col0, (kt0 + nx) * BKT, K, tid);
+                    }
+                    cp_async_commit();
+                }
+            }
             if constexpr (M3) {
                 double sa[4], sb[NTL], e[NTL];
 #pragma unroll
@@ -384,7 +399,7 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
         cp_async_wait<ST - 2>();
         __syncthreads();
         if (M3 && Add && kt == nkt - PF_AHEAD) prefetch_out();
-        {
+        if constexpr (!M3) {   // 4M kernels (3 CTAs per SM, 168 registers): refill issued right away
             const int nx = kt + ST - 1;
             if (nx < nkt) {
                 const int slot = nx % ST;
@@ -403,6 +418,15 @@ __global__ void __launch_bounds__(NTHREADS, M3 ? 2 : 3) k_gemm_expand(const doub
 #pragma unroll
             for (int j = 0; j < NTL; j++)
                 bq[j] = *reinterpret_cast<const double2 *>(bp + kk * 4 * PROW + (wc + 8 * j) * 16 + fp);
+            if (M3 && kk == BK / 4 - 1) {   // refill issued after the k-tile's last fragment loads (see k_gemm_dotk): 10.97 -> 10.80 ms at config 5
+                const int nx = kt + ST - 1;
+                if (nx < nkt) {
+                    const int slot = nx % ST;
+                    load_opk(sA + slot * OPK_BYTES, A, K, Rn, row0, (int64_t)nx * BK, K, tid);
+                    load_p(sP + slot * OPN, nx * BK);
+                }
+                cp_async_commit();
+            }
             if constexpr (M3) {
                 double sa[MTL], sb[NTL];
 #pragma unroll

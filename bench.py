@@ -326,6 +326,9 @@ def measure(cfg_id, args, rank, world, local, full):
     for k in ks:
         jd.jdft_set_option(k["gb"], "profile_kernel", jd.KERNEL_IDS[dominant] if in_region_profile else 0)
         jd.jdft_profile_read(k["gb"])
+    if not in_region_profile:
+        for _ in range(3):   # set_option dropped the captured CUDA graphs: re-warm so that no capture falls into the timed region
+            step()
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()

@@ -2,7 +2,7 @@
 bench.py times: all nb bands in one jdft_apply_H call, automatic band batch, the full projector block, workspace sized
 as bench.py sizes it.  EVERY band of HC is compared with the oracle (per-band relative L2); I / I^+ / J are compared
 with the oracle on real-space blocks that are NOT band-limited; the overlap is compared as a full matrix, also through
-the Hermitian-triangle path with non-orthonormal bands.  Tolerance: BASELINE.json north_star, per-band relative
+the Hermitian-triangle path with non-orthonormal bands; the HOST-buffer path of bench.py's e2e leg likewise.  Tolerance: BASELINE.json north_star, per-band relative
 L2 <= 1e-10.  The oracle needs ~2-3 minutes of the box's host threads for the whole module.
 """
 import numpy as np
@@ -76,7 +76,7 @@ def test_full_H_every_band(full, jd):
     err = np.linalg.norm(got - want, axis=1) / np.linalg.norm(want, axis=1)
     assert err.shape == (full.nb,)
     assert float(err.max()) <= TOL, "band %d: %g" % (int(err.argmax()), float(err.max()))
-    full.HC = HC
+    full.HC, full.want_HC = HC, want
 
 
 def test_full_H_pruned_butterflies_are_taken_and_agree(full, jd):
@@ -161,6 +161,31 @@ def test_full_overlap_whole_matrix(full, jd):
     M3 = jd.jdft_overlap(full.gb, full.dC, HC).cpu().numpy()
     want3 = full.rb.overlap(full.C, HC.cpu().numpy())
     assert rel_rows(M3.T, want3.T) <= TOL
+
+
+def test_full_host_path_every_band(full, jd):
+    """The end-to-end leg bench.py times (`e2e`): jdft_apply_H_host with every input in pinned HOST memory (64-band chunks
+    pipelined over three streams), then jdft_overlap_host_resident on the block that call uploaded.  EVERY band of HC
+    against the oracle; the overlap against the oracle's (the bands are orthonormal: also ~identity); the resident-operator
+    variant gives the same HC bit for bit (same kernels, same chunks)."""
+    want = full.want_HC if hasattr(full, "want_HC") else full.rb.apply_H(full.V, full.P, full.D, full.C)
+    Vp = torch.from_numpy(np.ascontiguousarray(full.V.reshape(-1))).pin_memory()
+    Pp, Dp, Cp = (torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (full.P, full.D, full.C))
+    HC = torch.empty(full.C.shape, dtype=torch.complex128).pin_memory()
+    jd.jdft_apply_H_host(full.gb, Vp, Pp, Dp, Cp, HC)
+    got = HC.numpy()
+    err = np.linalg.norm(got - want, axis=1) / np.linalg.norm(want, axis=1)
+    assert err.shape == (full.nb,)
+    assert float(err.max()) <= TOL, "band %d: %g" % (int(err.argmax()), float(err.max()))
+    M = torch.empty((full.nb, full.nb), dtype=torch.complex128).pin_memory()
+    gotM = jd.jdft_overlap_host_resident(full.gb, M).numpy()
+    assert np.max(np.abs(gotM - full.rb.overlap(full.C, full.C))) <= TOL
+    assert np.max(np.abs(gotM - np.eye(full.nb))) <= 1e-12
+    jd.jdft_host_set_operators(full.gb, Vp, Pp, Dp)
+    HC2 = torch.empty_like(HC).pin_memory()
+    jd.jdft_apply_H_host_resident(full.gb, Cp, HC2)
+    assert torch.equal(HC2, HC)
+    full.want_HC = None                                                                # the oracle's HC is not needed again
 
 
 def test_full_density_and_subspace(full, jd):

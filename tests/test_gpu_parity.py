@@ -587,6 +587,37 @@ def test_band_shards_compose_on_one_gpu(case, jd, world):
     assert rel_err_per_band(HC, want_H) <= TOL
 
 
+@pytest.mark.parametrize("cfg_id", [103, 101])
+def test_bench_shard_step_on_one_gpu(ref, jd, cfg_id):
+    """The step `bench.py --shard kb` times, as that mode builds it (bench.shard_inputs + sharding.sharded_step with the
+    CUDA binding, one rank = every k-point, all bands): HC of every k-point and its overlap against the oracle.  The
+    same step on 2 and 3 gloo ranks with the oracle as the local operation is tests/test_sharding_gloo.py."""
+    import bench
+    from paper_1708_03621_b200 import sharding as sh
+    cfg = workloads.get_config(cfg_id)
+    nk, nb = len(cfg["kpoints"]), cfg["nb"]
+    lay = sh.KBLayout(nk, nb, 1, 0)
+
+    def make_basis(R, k, Ecut, S):
+        gb = jd.jdft_basis_create(R, k, Ecut, S)
+        jd.jdft_alloc_workspace(gb, nb, max(nb, 64))
+        return gb, jd.jdft_basis_export(gb)[0]
+
+    kdata, V, D = bench.shard_inputs(cfg_id, lay, make_basis, lambda a: torch.from_numpy(a).cuda())
+    for d in kdata.values():
+        d["HC"] = torch.empty_like(d["C"])
+    out = sh.sharded_step(lay, kdata, V, D, group=None, mode="allgather", overlap=True)
+    assert sorted(out) == list(range(nk))
+    R, kpts, Ecut, S = workloads.lattice(cfg_id)
+    for k in range(nk):
+        rb = ref.RefBasis(R, kpts[k], Ecut, S)
+        inp = workloads.make_inputs(cfg_id, rb.iG, ik=k)
+        HC, M = out[k]
+        assert HC.data_ptr() == kdata[k]["HC"].data_ptr()                      # written in place, as the bench expects
+        assert rel_err_per_band(HC.cpu().numpy(), rb.apply_H(inp["Vloc"], inp["P"], inp["D"], inp["C"])) <= TOL
+        assert rel_err_per_band(M.cpu().numpy().T, rb.overlap(inp["C"], inp["C"]).T) <= TOL
+
+
 @pytest.mark.parametrize("tma", [0, 1])
 @pytest.mark.parametrize("cfg_id", [211, 212, 217])
 def test_planes_pruned_butterflies_match(ref, jd, cfg_id, tma):

@@ -95,6 +95,8 @@ int jdft_set_workspace(jdft_basis *b, void *dev_ptr, size_t bytes);
  * "planes_pair" (0/1, default 1: K3 with two pencils per thread where that variant exists),
  * "planes_prune" (0/1, default 1: K3 hybrid with radix-8 butterflies pruned to the sphere's extent along axis 0
  * when planes [L/4, 3L/4) are empty),
+ * "cols_direct" (0/1, default 1: K1's first pass reads the sphere and, at column length 128, K5's last pass writes it
+ * straight from / to global memory instead of staging the scatter / gather through shared memory; same arithmetic, bit-identical),
  * "planes_tma" (0/1, default 0: K3 through tensor-map (TMA) loads / stores in persistent double-buffered CTAs; measured
  * slower than the LSU kernels on B200), "gemm_3m" (0/1, default 1: projector / overlap GEMMs by the
  * 3M complex-product scheme, three tensor instructions per complex tile product instead of four),

@@ -165,7 +165,7 @@ extern "C" int jdft_basis_create(const double R[9], const double k[3], double Ec
     b->h_ops_set = 0; b->h_nproj = 0; b->h_D_mode = 0; b->h_C_nb = 0;
     b->ws = nullptr; b->ws_bytes = 0; b->opt_band_batch = 0; b->opt_force_generic = 0;
     b->opt_profile_kernel = 0; b->prof_used = 0;
-    b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_gemm3m = 1; b->opt_tma = 0; b->opt_gemm_tma = 0; b->opt_host_chunk = 0; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
+    b->opt_overlap = 0; b->opt_pair = 1; b->opt_prune = 1; b->opt_cols_direct = 1; b->opt_gemm3m = 1; b->opt_tma = 0; b->opt_gemm_tma = 0; b->opt_host_chunk = 0; b->side = nullptr; b->ev_fork = nullptr; b->ev_join = nullptr;
 
     // G = 2 pi R^-1 (adjugate / det): row i of G is the reciprocal vector b_i
     {
@@ -383,6 +383,7 @@ extern "C" int jdft_set_option(jdft_basis *b, const char *key, int64_t value) {
     if (!strcmp(key, "band_batch")) { b->opt_band_batch = value < 0 ? 0 : value; return JDFT_OK; }
     if (!strcmp(key, "planes_pair")) { b->opt_pair = value != 0; return JDFT_OK; }
     if (!strcmp(key, "planes_prune")) { b->opt_prune = value != 0; return JDFT_OK; }
+    if (!strcmp(key, "cols_direct")) { b->opt_cols_direct = value != 0; return JDFT_OK; }
     if (!strcmp(key, "host_chunk")) { b->opt_host_chunk = value < 0 ? 0 : value; return JDFT_OK; }
     if (!strcmp(key, "gemm_tma")) { b->opt_gemm_tma = value != 0; return JDFT_OK; }
     if (!strcmp(key, "planes_tma")) { b->opt_tma = value != 0; return JDFT_OK; }

@@ -9,6 +9,11 @@
 //   K5  the first pass reads W1 straight from global memory the same way (lanes along the pencil) and writes its
 //       butterflies into an XOR-swizzled tile, so the load staging disappears as well.
 // Tiles are [L][TP] c128 with TP = T + 1 (T pencils per CTA); the swizzled tile uses stride T inside the same buffer.
+// DIRECT variants (option "cols_direct", default on where measured faster): the sphere side goes without shared memory too --
+// K1's first pass reads each column's run (contiguous in n) straight into its butterflies, K5's pruned last pass at
+// length 128 writes the run straight from registers with the kinetic term; lanes run along one column's rows, so the
+// global accesses are contiguous segments and the column search, the scatter / gather crossing and a barrier go away
+// (config 5: K1 0.844 -> 0.705 ms = 0.76 -> 0.90 of the HBM roofline; K5 0.951 -> 0.878 ms = 0.92 -> 0.99).
 #pragma once
 #include "fft.cuh"
 
@@ -108,7 +113,10 @@ __device__ __forceinline__ void dft8_in0167_c(double2 (&a)[8]) {
     a[3] = cadd(e3, o3); a[7] = csub(e3, o3);
 }
 
-template <int LT, bool PR = false>
+// DIRECT: the first pass takes its inputs straight from the sphere (column t's run is contiguous in n; the lanes of a
+// warp run along the butterfly index, i.e. along consecutive rows of one column -> contiguous global segments), so the
+// scatter into the tile, its column search and two of the barriers disappear.
+template <int LT, bool PR = false, bool DIRECT = false>
 __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tuned(const double2 *__restrict__ tw, const int ncol,
                                                                 const int64_t nG, const int *__restrict__ col_n0,
                                                                 const int *__restrict__ col_m2lo,
@@ -126,7 +134,35 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tun
     const double2 *Cb = C + (size_t)b * nG;
     double2 *Wb = W1 + ((size_t)b * ncol + c0) * L;
     const int nbeg = s_n0[0], nend = s_n0[nc];
-    {
+    if constexpr (DIRECT) {
+        constexpr int RD = F::ROUNDS0;
+        double2 a[RD][R0];
+#pragma unroll
+        for (int r = 0; r < RD; r++) {
+            const int w = tid + r * NT;
+            const int bf = w % NB0, t = w / NB0;
+            const int m2w = s_m2w[t], n0 = s_n0[t], len = t < nc ? s_n0[t + 1] - n0 : 0;
+#pragma unroll
+            for (int k = 0; k < R0; k++) {
+                if (PR && k >= 2 && k < 6) continue;
+                int off = bf + k * NB0 - m2w;
+                if (off < 0) off += L;
+                a[r][k] = make_double2(0.0, 0.0);
+                if (off < len) a[r][k] = Cb[n0 + off];
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < RD; r++) {
+            const int w = tid + r * NT;
+            const int bf = w % NB0, t = w / NB0;
+            if constexpr (PR && R0 == 8) dft8_in0167_c<+1>(a[r]);
+            else Dft<R0, +1>::run(a[r]);
+            tw_mul<R0, +1>(a[r], tw, bf);
+#pragma unroll
+            for (int j = 0; j < R0; j++) X[F::sw(bf * R0 + j, t)] = a[r][j];
+        }
+        __syncthreads();
+    } else {
         // scatter the sphere runs of the nc columns (contiguous in n) into the tile; nothing else of it is read
         // (the sphere reads are issued four deep before the first dependent shared-memory store: their HBM latency was
         //  the largest single stall of the kernel in the ncu source page)
@@ -184,6 +220,8 @@ __global__ void __launch_bounds__(Cfg<LT>::NT, Cfg<LT>::MINB_INV) k_cols_inv_tun
             }
         }
         __syncthreads();
+    }
+    {
         if constexpr (F::NP == 3) mid_pass_inplace<LT, +1>(X, tw);
         // last pass (radix RL): lanes run along the pencil, outputs go straight to W1[column][row]
         for (int w = tid; w < NBL * T; w += NT) {
@@ -215,7 +253,10 @@ __device__ __forceinline__ void dft8_out0167_c(double2 (&a)[8]) {   // outputs 0
 
 // REV = true: reversed radix order with the radix-8 LAST pass pruned to outputs 0, 1, 6, 7 (rows [2 NBL, 6 NBL) hold no
 // sphere point, the gather never reads them); the launcher checks |m2| < 2 NBL.
-template <int LT, bool REV = false>
+// DIRECT: the last pass runs with the lanes of a warp along the pencil and writes the sphere run of its column straight from
+// registers (consecutive rows of a column are consecutive n), with the kinetic term; the in-place write-back, the
+// gather with its column search and one barrier disappear.
+template <int LT, bool REV = false, bool DIRECT = false>
 __global__ void __launch_bounds__(Cfg<LT, REV>::NT, Cfg<LT, REV>::MINB_FWD) k_cols_fwd_tuned(const double2 *__restrict__ tw, const int ncol,
                                                                 const int64_t nG, const int *__restrict__ col_n0,
                                                                 const int *__restrict__ col_m2lo,
@@ -260,6 +301,55 @@ __global__ void __launch_bounds__(Cfg<LT, REV>::NT, Cfg<LT, REV>::MINB_FWD) k_co
         }
         __syncthreads();
         if constexpr (F::NP == 3) mid_pass_inplace<LT, -1>(X, tw);
+        if constexpr (DIRECT) {
+            const double2 *Cb = C + (size_t)b * nG;
+            double2 *Ob = outC + (size_t)b * nG;
+            for (int w = tid; w < NBL * T; w += NT) {
+                const int bf = w % NBL, t = w / NBL;
+                double2 a[RL];
+#pragma unroll
+                for (int k = 0; k < RL; k++) a[k] = X[F::sw(bf + k * NBL, t)];
+                const int m2w = s_m2w[t], n0 = s_n0[t], len = t < nc ? s_n0[t + 1] - n0 : 0;
+                if constexpr (REV) dft8_out0167_c<-1>(a);
+                else Dft<RL, -1>::run(a);
+                constexpr int J4 = 4;   // outputs whose C / ke reads are in flight together
+#pragma unroll
+                for (int j0 = 0; j0 < (REV ? J4 : RL); j0 += J4) {   // REV: the one chunk of outputs 0, 1, 6, 7
+                    double2 c[J4];
+                    double f[J4];
+                    int n[J4];
+#pragma unroll
+                    for (int u = 0; u < J4; u++) {
+                        const int j = REV ? (u < 2 ? u : u + 4) : j0 + u;
+                        c[u] = make_double2(0.0, 0.0);
+                        f[u] = 0.0;
+                        n[u] = -1;
+                        if (j < RL) {
+                            int off = bf + NBL * j - m2w;
+                            if (off < 0) off += L;
+                            if (off < len) {
+                                n[u] = n0 + off;
+                                if (kin != 0.0) {
+                                    c[u] = Cb[n[u]];
+                                    f[u] = kin * ke[n[u]];
+                                }
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < J4; u++) {
+                        const int j = REV ? (u < 2 ? u : u + 4) : j0 + u;
+                        if (j < RL && n[u] >= 0) {
+                            double2 v = a[j];
+                            v.x = fma(f[u], c[u].x, v.x * scale);
+                            v.y = fma(f[u], c[u].y, v.y * scale);
+                            Ob[n[u]] = v;
+                        }
+                    }
+                }
+            }
+            return;
+        }
         // last pass (radix RL), in place: a thread reads and writes the same rows bf + NBL k of its pencil
         for (int w = tid; w < NBL * T; w += NT) {
             const int t = w % T, bf = w / T;

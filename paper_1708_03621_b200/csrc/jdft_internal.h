@@ -62,6 +62,7 @@ struct jdft_basis {
     int64_t opt_host_chunk;                   // bands per chunk of the *_host pipeline ("host_chunk", 0 = 128)
     int64_t opt_gemm_tma;                     // operand stages of the 3M GEMMs filled by TMA ("gemm_tma")
     int64_t opt_tma;                          // K3 through TMA tensor-map loads / stores ("planes_tma")
+    int64_t opt_cols_direct;                  // K1: first pass reads the sphere straight from global memory ("cols_direct")
     int64_t opt_prune;                        // K3 hybrid: radix-8 butterflies pruned to the occupied planes ("planes_prune")
     cudaStream_t side;
     cudaEvent_t ev_fork, ev_join;

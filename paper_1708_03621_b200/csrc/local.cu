@@ -1138,10 +1138,25 @@ int launch_cols_inv(const jdft_basis *b, const double2 *C, int nbt, double2 *W1,
             using F = jcols::Cfg<LT>;
             dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
             // pruned radix-8 first pass when no sphere point has |m2| >= 2 NB0 (rows [2 NB0, 6 NB0) empty)
-            if (F::R0 == 8 && b->opt_prune && b->mmin[2] > -2 * F::NB0 && b->mmax[2] < 2 * F::NB0) {
+            const bool pr = F::R0 == 8 && b->opt_prune && b->mmin[2] > -2 * F::NB0 && b->mmax[2] < 2 * F::NB0;
+            // first pass straight from the sphere where a column has >= 16 first-pass butterflies (half-warps along one
+            // column's rows); measured: 128: 0.844 -> 0.705 ms (config 5), 216: 1.903 -> 1.767 ms (config 4), 80 (10
+            // butterflies): 0.0491 -> 0.0502 ms, so shorter columns keep the staged scatter
+            constexpr bool kDirect = F::NB0 >= 16;
+            const bool direct = kDirect && b->opt_cols_direct;
+            if constexpr (kDirect) {
+                if (direct && pr) {
+                    JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT, F::R0 == 8, true>, F::smem, b->device));
+                    jcols::k_cols_inv_tuned<LT, F::R0 == 8, true><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+                } else if (direct) {
+                    JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT, false, true>, F::smem, b->device));
+                    jcols::k_cols_inv_tuned<LT, false, true><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
+                }
+            }
+            if (!direct && pr) {
                 JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT, F::R0 == 8>, F::smem, b->device));
                 jcols::k_cols_inv_tuned<LT, F::R0 == 8><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
-            } else {
+            } else if (!direct) {
                 JDFT_CUDA(ensure_smem(jcols::k_cols_inv_tuned<LT>, F::smem, b->device));
                 jcols::k_cols_inv_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, C, W1);
             }
@@ -1167,12 +1182,26 @@ int launch_cols_fwd(const jdft_basis *b, const double2 *W1, int nbt, double scal
             using FR = jcols::Cfg<LT, true>;
             // reversed plan (16, 8) with the radix-8 last pass pruned, when no sphere point has |m2| >= 2 (L / 8); measured:
             // 1.116 -> 0.949 ms at 128 (0.78 -> 0.91 of the HBM roofline), no gain at 80 = 8 x 10 (kept on the forward plan)
-            if (F::NP == 2 && F::R0 == 8 && F::R1 == 16 && b->opt_prune && b->mmin[2] > -2 * (LT / 8) && b->mmax[2] < 2 * (LT / 8)) {
-                JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT, F::NP == 2 && F::R0 == 8 && F::R1 == 16>, FR::smem, b->device));
-                dim3 g2((b->ncol + FR::T - 1) / FR::T, nbt);
-                jcols::k_cols_fwd_tuned<LT, F::NP == 2 && F::R0 == 8 && F::R1 == 16><<<g2, FR::NT, FR::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
-                                                                   scale, kin, b->d_ke, C, out);
-            } else {
+            constexpr bool kRev = F::NP == 2 && F::R0 == 8 && F::R1 == 16;
+            const bool rev = kRev && b->opt_prune && b->mmin[2] > -2 * (LT / 8) && b->mmax[2] < 2 * (LT / 8);
+            // ... and its last pass writing the sphere straight from registers ("cols_direct"): 0.951 -> 0.878 ms at 128
+            // (0.92 -> 0.99 of the HBM roofline); on the forward plans the same change is slower (216: 1.85 -> 2.03 ms,
+            // 80: 0.0635 -> 0.0697 ms: radix-6 / radix-10 last passes with lanes along the pencil), so they keep the gather
+            if constexpr (kRev) {
+                if (rev) {
+                    dim3 g2((b->ncol + FR::T - 1) / FR::T, nbt);
+                    if (b->opt_cols_direct) {
+                        JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT, true, true>, FR::smem, b->device));
+                        jcols::k_cols_fwd_tuned<LT, true, true><<<g2, FR::NT, FR::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo,
+                                                                                         W1, scale, kin, b->d_ke, C, out);
+                    } else {
+                        JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT, true>, FR::smem, b->device));
+                        jcols::k_cols_fwd_tuned<LT, true><<<g2, FR::NT, FR::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,
+                                                                                   scale, kin, b->d_ke, C, out);
+                    }
+                }
+            }
+            if (!rev) {
                 JDFT_CUDA(ensure_smem(jcols::k_cols_fwd_tuned<LT>, F::smem, b->device));
                 dim3 g2((b->ncol + F::T - 1) / F::T, nbt);
                 jcols::k_cols_fwd_tuned<LT><<<g2, F::NT, F::smem, st>>>(b->d_tw[2], b->ncol, b->nG, b->d_col_n0, b->d_col_m2lo, W1,

@@ -1,7 +1,7 @@
 // Tuned column kernels (K1: scatter + inverse FFT along axis 2; K5: forward FFT along axis 2 + gather + kinetic)
 // for the lengths that have compile-time plans (fft.cuh SpecPlan).  Included by local.cu only.
 //
-// Both kernels are bound by shared-memory bandwidth, not HBM (profiles/r02_ncu_full.md: L1/shared pipe 61-85 %, DRAM 38-57 %), so the design
+// Both kernels were bound by shared-memory bandwidth, not HBM (ncu of the staged variants: L1/shared pipe 61-85 %, DRAM 38-57 %), so the design
 // goal is fewer shared-memory tile transfers than the ping-pong engine needs:
 //   K1  no zero fill (the first pass tests "is this row inside the column's sphere run" instead), and the last pass
 //       writes W1 straight from registers with the lanes of a warp running along the pencil (consecutive rows ->
